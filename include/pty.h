@@ -1,0 +1,175 @@
+/* pty.h -- C ABI of the B200-native (sm_100a) multislice-ptychography hot path.
+ *
+ * What it computes: the batched mixed-state multislice forward model of PtyRAD
+ * (arxiv 2505.07814; PAPER.md = /root/reference/PAPER.md), an amplitude loss and the
+ * exact hand-written adjoint over one minibatch of B scan positions:
+ *
+ *   r_b = floor(p_b + 0.5),  Delta_b = p_b - r_b                  (footnote 3 :122)
+ *   psi_0^(m) = F^-1[ exp(-2 pi i k.Delta_b) F[P^(m)] ]           (shift operator)
+ *   for s = 1..Nz:  phi_s = O[s, r_b : r_b+N] * psi_{s-1};
+ *                   psi_s = F^-1[ M F[phi_s] ]  for s < Nz         (Eq. 3)
+ *   M(k) = exp(-i pi lambda |k|^2 dz + 2 pi i dz (k_x tan th_x + k_y tan th_y))   (Eq. 4, :89)
+ *   I_b(k) = sum_m |F[phi_Nz^(m)](k)|^2                           (Eq. 2)
+ *   L = sum_b sum_k (sqrt(I_b(k)) - a_b(k))^2                     (Eq. 5 with p = 1/2, :126-131;
+ *                                                                  plain sum, R13)
+ * F is the unitary 2-D DFT with kernel exp(-2 pi i k.r); k = fftfreq(N)/dx in 1/Angstrom.
+ * Gradients use g = dL/dRe + i dL/dIm for complex arrays (what torch.autograd returns);
+ * g_positions = dL/dDelta (the integer crop origin is a constant).
+ *
+ * Layouts.  Every array is dense, row-major, C order, exactly as named below; complex means
+ * interleaved (re, im) float32 ("c64").  2-D arrays are (y, x); spectra / detector data have
+ * DC at index [0][0] (unshifted FFT order).  positions[b] = (p_y, p_x) in PIXELS = the top-left
+ * corner of the N x N crop in object coordinates.  tilt = (theta_y, theta_x) in RADIANS.
+ *
+ * Memory.  Unless a parameter says "host", every pointer is a DEVICE pointer on the plan's
+ * device.  The caller owns every buffer including the workspace and the Adam moments; the
+ * library allocates no device memory, frees nothing of the caller's and keeps no caller pointer
+ * past a call (except the workspace given to pty_create).
+ *
+ * Execution.  Everything is enqueued on the given stream; no call synchronises except
+ * pty_status and the *_host entry points.  One plan per stream; a plan is not thread-safe.
+ *
+ * Errors.  Every function returns PTY_OK (0) or a negative PTY_ERR_* code; the text of the last
+ * error of a plan is available from pty_last_error.  No C++ exception crosses this boundary.
+ * Scan positions are device data: a crop that would leave the object is clamped into it and a
+ * sticky device flag is raised, reported by pty_status as PTY_ERR_BOUNDS.
+ * There is no CPU fallback of any kind.
+ */
+#ifndef PTY_H
+#define PTY_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PTY_OK                 0
+#define PTY_ERR_INVALID_ARG   (-1)  /* null pointer, B < 0 or B > Bmax, bad dims            */
+#define PTY_ERR_UNSUPPORTED   (-2)  /* N not in {64,128,256}, window larger than the object   */
+#define PTY_ERR_WORKSPACE     (-3)  /* workspace null, misaligned (256 B) or too small        */
+#define PTY_ERR_CUDA          (-4)  /* a CUDA runtime call failed; see pty_last_error         */
+#define PTY_ERR_BOUNDS        (-5)  /* pty_status: some crop left the object and was clamped  */
+
+/* pty_dims.flags */
+#define PTY_FLAG_SPECTRA       1    /* keep propagated spectra so that g_dz can be produced even
+                                       when tilt_mode == 0 (implied by tilt_mode != 0)        */
+#define PTY_FLAG_STEP          2    /* reserve gradient buffers in the workspace: pty_step     */
+#define PTY_FLAG_HOST          4    /* reserve device staging buffers: pty_grad_host           */
+
+/* pty_backward flags */
+#define PTY_BWD_ACCUMULATE     1    /* add into the gradient outputs instead of overwriting    */
+#define PTY_BWD_RECOMPUTE      2    /* do not trust the state left by pty_forward_loss         */
+
+typedef struct pty_plan pty_plan;   /* opaque, host side */
+
+typedef struct pty_dims {
+    int32_t Nz, H, W;     /* object [Nz][H][W] c64                                            */
+    int32_t M, N;         /* probe  [M][N][N] c64; N in {64, 128, 256}; N <= H, N <= W        */
+    int32_t Bmax;         /* largest minibatch any call will pass                             */
+    float   dz, lambda, dx;   /* slice separation, wavelength, pixel size; Angstrom (Eq. 4)   */
+    int32_t tilt_mode;    /* 0: no tilt (tilt pointers ignored); 1: one global tilt [2];
+                             2: one tilt per position [B][2]                                  */
+    int32_t flags;        /* PTY_FLAG_*                                                       */
+} pty_dims;
+
+/* Adam hyper-parameters (Kingma & Ba with bias correction; R20).
+ * A learning rate of 0 freezes that parameter group (its moments are left untouched). */
+typedef struct pty_adam {
+    float lr_object, lr_probe, lr_positions, lr_tilt;
+    float beta1, beta2, eps;
+    int32_t t;            /* 1-based step number used for the bias correction                 */
+} pty_adam;
+
+/* Adam moments, device memory owned by the caller, float32, same element order as the
+ * parameter viewed as reals (complex = 2 floats).  A group with lr == 0 may pass NULL. */
+typedef struct pty_adam_state {
+    float *m_object,    *v_object;     /* [Nz*H*W*2] */
+    float *m_probe,     *v_probe;      /* [M*N*N*2]  */
+    float *m_positions, *v_positions;  /* [B*2]      */
+    float *m_tilt,      *v_tilt;       /* [2] (tilt_mode 1) or [B*2] (tilt_mode 2) */
+} pty_adam_state;
+
+/* Bytes of device workspace a plan with these dims needs (a multiple of 256). */
+int pty_workspace_bytes(const pty_dims* dims, size_t* out_bytes);
+
+/* Create a plan on `device` using the caller's device workspace (256-byte aligned, at least
+ * pty_workspace_bytes).  The workspace must stay alive and untouched until pty_destroy. */
+int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_t workspace_bytes,
+               int device);
+int pty_destroy(pty_plan* plan);
+
+/* Forward model + loss for one minibatch (PAPER.md:58-90 Eq. 1-4, :126-131 Eq. 5).
+ *   object [Nz][H][W] c64, probe [M][N][N] c64, positions [B][2] f32, tilt per tilt_mode
+ *   (may be NULL when tilt_mode == 0), meas_amp [B][N][N] f32 = sqrt(counts), DC at [0][0].
+ * Outputs (device):
+ *   loss          [1] f64      = L                                   (required)
+ *   loss_per_pos  [B] f32      = sum_k (sqrt(I_b) - a_b)^2           (may be NULL)
+ *   intensity     [B][N][N] f32 = I_b(k)                             (may be NULL)
+ * Leaves the incident waves of every slice in the workspace for pty_backward. */
+int pty_forward_loss(pty_plan* plan, const void* object, const void* probe,
+                     const float* positions, const float* tilt, const float* meas_amp, int32_t B,
+                     double* loss, float* loss_per_pos, float* intensity, void* stream);
+
+/* Exact gradient of L for the same minibatch (hand-written adjoint).
+ * Uses the state left by the immediately preceding pty_forward_loss on this plan when that call
+ * had the same pointers and B; otherwise (or with PTY_BWD_RECOMPUTE) it runs the forward itself.
+ * Outputs (device; any may be NULL = not wanted, except g_object):
+ *   g_object    [Nz][H][W] c64  scatter-add over the overlapping patches
+ *   g_probe     [M][N][N] c64
+ *   g_positions [B][2] f32      = dL/dDelta_b  (y, x)
+ *   g_tilt      [2] (tilt_mode 1: summed over b) or [B][2] (tilt_mode 2); ignored for mode 0
+ *   g_dz        [1] f32         = dL/d(dz); needs tilt_mode != 0 or PTY_FLAG_SPECTRA
+ * flags: PTY_BWD_ACCUMULATE, PTY_BWD_RECOMPUTE. */
+int pty_backward(pty_plan* plan, const void* object, const void* probe,
+                 const float* positions, const float* tilt, const float* meas_amp, int32_t B,
+                 void* g_object, void* g_probe, float* g_positions, float* g_tilt, float* g_dz,
+                 int32_t flags, void* stream);
+
+/* One optimisation step: forward, loss, gradient and an Adam update of object, probe, positions
+ * and tilt in place (plan needs PTY_FLAG_STEP).  loss [1] f64 device = L before
+ * the update.  hp and st are HOST structs (st holds device pointers). */
+int pty_step(pty_plan* plan, void* object, void* probe, float* positions, float* tilt,
+             const float* meas_amp, int32_t B, const pty_adam* hp, const pty_adam_state* st,
+             double* loss, void* stream);
+
+/* Adam update of one flat float32 parameter array (the kernel pty_step uses), exposed for
+ * callers that keep their own gradient buffers.  All device pointers, n floats. */
+int pty_adam_update(pty_plan* plan, float* theta, const float* grad, float* m, float* v, size_t n,
+                    float lr, float beta1, float beta2, float eps, int32_t t, void* stream);
+
+/* End-to-end variant with HOST buffers (pinned memory recommended; plan needs PTY_FLAG_HOST):
+ * copies the inputs host->device, runs pty_forward_loss + pty_backward, copies loss and the
+ * gradients device->host and synchronises the stream before returning.  Host outputs that are
+ * NULL are skipped. */
+int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe,
+                  const float* h_positions, const float* h_tilt, const float* h_meas_amp, int32_t B,
+                  double* h_loss, void* h_g_object, void* h_g_probe, float* h_g_positions,
+                  float* h_g_tilt, void* stream);
+
+/* Synchronises the plan's last stream and returns PTY_OK, PTY_ERR_BOUNDS or PTY_ERR_CUDA.
+ * device_flags (host, may be NULL) receives the raw sticky flag word and clears it. */
+int pty_status(pty_plan* plan, int32_t* device_flags);
+
+/* Kernel timing for benchmarks.  pty_profile(plan, 1) makes every later call bracket its forward
+ * (a2-a5) and adjoint (a7-a13) kernel launches with CUDA events on the call's own stream (at most
+ * 1024 launches are kept; older ones are dropped); pty_profile(plan, 0) stops and forgets them.
+ * pty_profile_read synchronises the plan's stream and returns, for the launches recorded since the
+ * last read, the summed device time in milliseconds and the launch count of each kernel (host out). */
+int pty_profile(pty_plan* plan, int32_t enable);
+int pty_profile_read(pty_plan* plan, float* fwd_ms, int32_t* fwd_launches, float* bwd_ms, int32_t* bwd_launches);
+
+/* Number of kernel launches the plan has enqueued so far (for bench accounting). */
+int64_t pty_launch_count(const pty_plan* plan);
+
+/* Text of the plan's last error ("" if none).  plan == NULL returns the last creation error. */
+const char* pty_last_error(const pty_plan* plan);
+
+/* Library version string, e.g. "pty-b200 0.1 (sm_100a)". */
+const char* pty_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PTY_H */

@@ -1,0 +1,204 @@
+// pty_fft.cuh -- register butterflies and the shared-memory line-FFT passes.
+//
+// A wave of N x N complex64 lives in shared memory as S[N][PITCH] (PITCH odd).  One "pass" is a
+// 1-D FFT over the SLOW index (rows) for every line (column), done in two register stages
+// (N = R1*R2, decimation in time) and written back TRANSPOSED, so that the next pass again
+// transforms over the slow index.  Two passes = one 2-D FFT, and the wave is back in (y, x)
+// orientation.  Lanes of a warp always run along the line index: shared-memory reads are
+// lane-contiguous, transposed writes hit stride PITCH (odd) -> conflict-free for 8-byte words.
+// For N = 256 the N lines are split over a cluster of CL = 4 CTAs (64 lines each); the
+// transposed write then goes to the owning CTA's shared memory through DSMEM.
+//
+//   X[k1 + R1 k2] = sum_{n2} W_N^{n2 k1} W_{R2}^{n2 k2} [ sum_{n1} x[R2 n1 + n2] W_{R1}^{n1 k1} ]
+//
+// DIR = -1: forward kernel exp(-2 pi i nk/N);  DIR = +1: inverse (unscaled).
+#pragma once
+#ifndef PTY_PORT_INCLUDED
+#include "pty_port.cuh"
+#endif
+
+namespace pty {
+
+// ----------------------------------------------------------------------------- complex helpers
+PTY_DEV float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+PTY_DEV float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+PTY_DEV float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// conj(a) * b
+PTY_DEV float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }
+PTY_DEV float2 cscale(float2 a, float s) { return make_float2(a.x * s, a.y * s); }
+PTY_DEV float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
+
+// a * exp(DIR * i * pi/2): forward multiplies by -i, inverse by +i
+template <int DIR> PTY_DEV float2 mul_qi(float2 a) {
+    return DIR < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+}
+// a * (c + i*DIR*s) with c, s the cos/sin of a positive angle
+template <int DIR> PTY_DEV float2 mul_cs(float2 a, float c, float s) {
+    return DIR < 0 ? make_float2(a.x * c + a.y * s, a.y * c - a.x * s)
+                   : make_float2(a.x * c - a.y * s, a.y * c + a.x * s);
+}
+
+// ----------------------------------------------------------------------------- radix-4 / 8 / 16
+template <int DIR> PTY_DEV void bfly4(float2& a0, float2& a1, float2& a2, float2& a3) {
+    float2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = mul_qi<DIR>(csub(a1, a3));
+    a0 = cadd(t0, t2); a2 = csub(t0, t2); a1 = cadd(t1, t3); a3 = csub(t1, t3);
+}
+
+template <int R, int DIR> struct RegFFT;
+
+template <int DIR> struct RegFFT<8, DIR> {
+    static PTY_DEV void run(float2 (&v)[8]) {
+        const float h = 0.70710678118654752440f;
+        bfly4<DIR>(v[0], v[2], v[4], v[6]);           // E_k at v[0],v[2],v[4],v[6]
+        bfly4<DIR>(v[1], v[3], v[5], v[7]);           // O_k at v[1],v[3],v[5],v[7]
+        float2 o1 = mul_cs<DIR>(v[3], h, h);          // W8^1
+        float2 o2 = mul_qi<DIR>(v[5]);                // W8^2
+        float2 o3 = mul_cs<DIR>(mul_qi<DIR>(v[7]), h, h);   // W8^3 = W8^2 W8^1
+        float2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+        v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+        v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
+        v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
+        v[3] = cadd(e3, o3); v[7] = csub(e3, o3);
+    }
+};
+
+template <int DIR> struct RegFFT<16, DIR> {
+    static PTY_DEV void run(float2 (&v)[16]) {
+        const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;   // pi/8
+        const float h = 0.70710678118654752440f;                                   // pi/4
+        // stage 1: 4-point DFTs over n1 for every n2 (inputs v[4 n1 + n2]); result k1 at v[4 k1 + n2]
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) bfly4<DIR>(v[n2], v[4 + n2], v[8 + n2], v[12 + n2]);
+        // twiddles W16^{n2 k1}
+        v[4 + 1] = mul_cs<DIR>(v[4 + 1], c1, s1);                  // k1=1,n2=1: W^1
+        v[4 + 2] = mul_cs<DIR>(v[4 + 2], h, h);                    // W^2
+        v[4 + 3] = mul_cs<DIR>(v[4 + 3], s1, c1);                  // W^3
+        v[8 + 1] = mul_cs<DIR>(v[8 + 1], h, h);                    // k1=2,n2=1: W^2
+        v[8 + 2] = mul_qi<DIR>(v[8 + 2]);                          // W^4
+        v[8 + 3] = mul_cs<DIR>(mul_qi<DIR>(v[8 + 3]), h, h);       // W^6 = W^4 W^2
+        v[12 + 1] = mul_cs<DIR>(v[12 + 1], s1, c1);                // k1=3,n2=1: W^3
+        v[12 + 2] = mul_cs<DIR>(mul_qi<DIR>(v[12 + 2]), h, h);     // W^6
+        v[12 + 3] = mul_cs<DIR>(mul_qi<DIR>(mul_qi<DIR>(v[12 + 3])), c1, s1);   // W^9 = W^8 W^1
+        // stage 2: 4-point DFTs over n2 for every k1; X[k1 + 4 k2] lands in v[4 k1 + k2]
+#pragma unroll
+        for (int k1 = 0; k1 < 4; ++k1) bfly4<DIR>(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);
+        // to natural order: out[k1 + 4 k2] = v[4 k1 + k2]  (a 4x4 transpose)
+        float2 t;
+        t = v[1]; v[1] = v[4]; v[4] = t;
+        t = v[2]; v[2] = v[8]; v[8] = t;
+        t = v[3]; v[3] = v[12]; v[12] = t;
+        t = v[6]; v[6] = v[9]; v[9] = t;
+        t = v[7]; v[7] = v[13]; v[13] = t;
+        t = v[11]; v[11] = v[14]; v[14] = t;
+    }
+};
+
+// ----------------------------------------------------------------------------- shapes
+template <int N_> struct Shape;
+template <> struct Shape<64>  { static constexpr int N = 64,  R1 = 8,  R2 = 8,  CL = 1, NL = 64,  NT = 256; };
+template <> struct Shape<128> { static constexpr int N = 128, R1 = 16, R2 = 8,  CL = 1, NL = 128, NT = 512; };
+template <> struct Shape<256> { static constexpr int N = 256, R1 = 16, R2 = 16, CL = 4, NL = 64,  NT = 512; };
+
+template <class SH> struct ShapeInfo {
+    static constexpr int N = SH::N, R1 = SH::R1, R2 = SH::R2, CL = SH::CL, NL = SH::NL, NT = SH::NT;
+    static constexpr int PITCH = NL + 1;
+    static constexpr int TA = (R2 * NL) / NT;      // stage-A tasks per thread
+    static constexpr int TB = (R1 * NL) / NT;      // stage-B tasks per thread
+    static constexpr int SWEEP = (N * NL) / NT;    // elements per thread in a sweep
+    static_assert(R1 * R2 == N, "radix split");
+    static_assert((R2 * NL) % NT == 0 && (R1 * NL) % NT == 0, "task split");
+    static_assert(NL % 32 == 0, "a warp must stay inside one task group");
+    static constexpr size_t wave_bytes = size_t(N) * PITCH * sizeof(float2);
+    static constexpr size_t table_bytes = size_t(5) * N * sizeof(float2) + 64 * sizeof(float);
+    static constexpr size_t smem_bytes = wave_bytes + table_bytes;
+};
+
+// Per-CTA view: thread id, rank in the cluster, the wave buffer of every CTA of the cluster
+// (Sr[rank] == S), the small tables.
+template <class SH> struct Cta {
+    int tid, rank;
+    float2* S;
+    float2* Sr[SH::CL];
+    float2 *tw, *Ey, *Ex, *My, *Mx;   // [N] each: twiddles exp(-2 pi i j/N); shift and propagator factors
+    float* red;                       // [64] block-reduction scratch
+};
+
+template <class SH> PTY_DEV void sync_all() {
+    if (SH::CL > 1) pty_cluster_sync(); else pty_cta_sync();
+}
+
+// ----------------------------------------------------------------------------- stage A
+// In::load(cta, n2, line, gline, v) fills v[n1] = element (row = R2 n1 + n2, line) of the input,
+// with whatever pointwise work is fused there (see pty_kernels.cuh).
+template <class SH, int DIR, class In>
+PTY_DEV void stage_a(const Cta<SH>& c, In& in) {
+    using I = ShapeInfo<SH>;
+#pragma unroll 1
+    for (int it = 0; it < I::TA; ++it) {
+        const int t = it * I::NT + c.tid;
+        const int line = t % I::NL, n2 = t / I::NL;
+        float2 v[I::R1];
+        in.load(c, n2, line, c.rank * I::NL + line, v);
+        RegFFT<I::R1, DIR>::run(v);
+#pragma unroll
+        for (int k1 = 1; k1 < I::R1; ++k1) {
+            float2 w = c.tw[n2 * k1];
+            if (DIR > 0) w.y = -w.y;
+            v[k1] = cmul(v[k1], w);
+        }
+#pragma unroll
+        for (int k1 = 0; k1 < I::R1; ++k1) c.S[(I::R2 * k1 + n2) * I::PITCH + line] = v[k1];
+    }
+}
+
+// ----------------------------------------------------------------------------- stage B
+// Reads everything into registers, synchronises, then writes the transposed result:
+// element (old line L_global, k) goes to row L_global, column k of the new orientation,
+// i.e. to CTA k / NL at Sr[.][L_global * PITCH + k % NL].
+template <class SH, int DIR>
+PTY_DEV void stage_b(const Cta<SH>& c) {
+    using I = ShapeInfo<SH>;
+    float2 v[I::TB][I::R2];
+#pragma unroll
+    for (int it = 0; it < I::TB; ++it) {
+        const int t = it * I::NT + c.tid;
+        const int line = t % I::NL, k1 = t / I::NL;
+#pragma unroll
+        for (int n2 = 0; n2 < I::R2; ++n2) v[it][n2] = c.S[(I::R2 * k1 + n2) * I::PITCH + line];
+        RegFFT<I::R2, DIR>::run(v[it]);
+    }
+    sync_all<SH>();
+#pragma unroll
+    for (int it = 0; it < I::TB; ++it) {
+        const int t = it * I::NT + c.tid;
+        const int line = t % I::NL, k1 = t / I::NL;
+        const int grow = c.rank * I::NL + line;
+#pragma unroll
+        for (int k2 = 0; k2 < I::R2; ++k2) {
+            const int k = k1 + I::R1 * k2;
+            float2* dst = (SH::CL > 1) ? c.Sr[k / I::NL] : c.S;
+            dst[grow * I::PITCH + (k % I::NL)] = v[it][k2];
+        }
+    }
+    sync_all<SH>();
+}
+
+// One full pass: stage A (with its fused input work), stage B, transposed write.
+template <class SH, int DIR, class In>
+PTY_DEV void fft_pass(const Cta<SH>& c, In& in) {
+    stage_a<SH, DIR>(c, in);
+    pty_cta_sync();
+    stage_b<SH, DIR>(c);
+}
+
+// Plain input: the wave itself.
+struct InSmem {
+    template <class SH, int R>
+    PTY_DEV void load(const Cta<SH>& c, int n2, int line, int, float2 (&v)[R]) {
+        using I = ShapeInfo<SH>;
+#pragma unroll
+        for (int n1 = 0; n1 < R; ++n1) v[n1] = c.S[(I::R2 * n1 + n2) * I::PITCH + line];
+    }
+};
+
+}  // namespace pty

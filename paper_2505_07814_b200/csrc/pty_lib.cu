@@ -1,0 +1,656 @@
+// pty_lib.cu -- __global__ entry points, the small per-call kernels and the C ABI of include/pty.h.
+// sm_100a only; no cuFFT, no CPU fallback: every step of the hot path runs in the kernels here.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/pty.h"
+#include "pty_kernels.cuh"
+
+namespace cg = cooperative_groups;
+using namespace pty;
+
+// ============================================================================ kernels
+template <class SH>
+__device__ __forceinline__ Cta<SH> make_cta(unsigned char* smem) {
+    using I = ShapeInfo<SH>;
+    Cta<SH> c;
+    c.tid = threadIdx.x;
+    c.rank = 0;
+    c.S = reinterpret_cast<float2*>(smem);
+    if constexpr (SH::CL > 1) {
+        cg::cluster_group cl = cg::this_cluster();
+        c.rank = (int)cl.block_rank();
+#pragma unroll
+        for (int k = 0; k < SH::CL; ++k) c.Sr[k] = cl.map_shared_rank(c.S, k);
+    } else {
+        c.Sr[0] = c.S;
+    }
+    float2* tab = reinterpret_cast<float2*>(smem + I::wave_bytes);
+    c.tw = tab; c.Ey = tab + SH::N; c.Ex = tab + 2 * SH::N; c.My = tab + 3 * SH::N; c.Mx = tab + 4 * SH::N;
+    c.red = reinterpret_cast<float*>(tab + 5 * SH::N);
+    return c;
+}
+
+template <class SH> struct MinBlocks { static constexpr int value = SH::N == 64 ? 2 : 1; };
+
+template <class SH>
+__global__ void __launch_bounds__(SH::NT, MinBlocks<SH>::value) pty_fwd_kernel(const KArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    Cta<SH> c = make_cta<SH>(smem);
+    if constexpr (SH::CL > 1) cg::this_cluster().sync();
+    fwd_body<SH>(A, c, blockIdx.x / SH::CL);
+}
+
+template <class SH>
+__global__ void __launch_bounds__(SH::NT, MinBlocks<SH>::value) pty_bwd_kernel(const KArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    Cta<SH> c = make_cta<SH>(smem);
+    if constexpr (SH::CL > 1) cg::this_cluster().sync();
+    bwd_body<SH>(A, c, blockIdx.x / SH::CL);
+}
+
+template <class SH, int DIR>
+__global__ void __launch_bounds__(SH::NT, MinBlocks<SH>::value)
+pty_fft2_kernel(const float2* src, float2* dst, float scale, int accumulate) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    Cta<SH> c = make_cta<SH>(smem);
+    if constexpr (SH::CL > 1) cg::this_cluster().sync();
+    fft2_body<SH, DIR>(src, dst, scale, accumulate, c, blockIdx.x / SH::CL);
+}
+
+// a0: separable propagator factors exp(i chi_y(k_y)), exp(i chi_x(k_x)) of Eq. 4 for one global tilt
+// (PAPER.md:89): chi_a(k) = -pi lambda dz k^2 + 2 pi dz k tan(theta_a), k = fftfreq(N)/dx.  Double
+// precision: 2N values per call.
+__global__ void pty_prop_table_kernel(int N, float dz, float lambda, float dx, const float* tilt,
+                                      float2* prop_y, float2* prop_x) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    const double ty = tilt ? (double)tilt[0] : 0.0, tx = tilt ? (double)tilt[1] : 0.0;
+    const double k = (double)(j < N / 2 ? j : j - N) / ((double)N * (double)dx);
+    const double quad = -3.14159265358979323846 * (double)lambda * (double)dz * k * k;
+    const double lin = 2.0 * 3.14159265358979323846 * (double)dz * k;
+    const double chy = quad + lin * tan(ty), chx = quad + lin * tan(tx);
+    prop_y[j] = make_float2((float)cos(chy), (float)sin(chy));
+    prop_x[j] = make_float2((float)cos(chx), (float)sin(chx));
+}
+
+// a6: L_b = sum_k (sqrt(I_b) - a_b)^2 (Eq. 5, p = 1/2, plain sum); one block per position.
+__global__ void __launch_bounds__(256) pty_loss_kernel(const float* __restrict__ I, const float* __restrict__ a,
+                                                       int NN, double* loss, float* loss_per_pos) {
+    const int b = blockIdx.x;
+    const float4* I4 = reinterpret_cast<const float4*>(I + (size_t)b * NN);
+    const float4* a4 = reinterpret_cast<const float4*>(a + (size_t)b * NN);
+    float acc = 0.f;
+    for (int i = threadIdx.x; i < NN / 4; i += blockDim.x) {
+        const float4 iv = __ldg(I4 + i), av = __ldg(a4 + i);
+        float d;
+        d = sqrtf(iv.x) - av.x; acc += d * d;
+        d = sqrtf(iv.y) - av.y; acc += d * d;
+        d = sqrtf(iv.z) - av.z; acc += d * d;
+        d = sqrtf(iv.w) - av.w; acc += d * d;
+    }
+    __shared__ double part[8];
+    double dacc = (double)acc;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dacc += __shfl_xor_sync(0xffffffffu, dacc, o);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = dacc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += part[w];
+        if (loss_per_pos) loss_per_pos[b] = (float)t;
+        atomicAdd(loss, t);
+    }
+}
+
+// a13 (B8): tilt and dz gradients from the per-position sums of D(k) (k in cycles/pixel).
+__global__ void pty_tilt_finalize_kernel(const float* dsum, const float* tilt, int B, int tilt_mode,
+                                         float dz, float lambda, float dx, float* g_tilt, float* g_dz,
+                                         int accumulate) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const double two_pi = 6.283185307179586476925;
+    double gty = 0.0, gtx = 0.0, gz = 0.0;
+    for (int b = 0; b < B; ++b) {
+        double ty = 0.0, tx = 0.0;
+        if (tilt_mode == 1) { ty = tilt[0]; tx = tilt[1]; }
+        if (tilt_mode == 2) { ty = tilt[2 * b]; tx = tilt[2 * b + 1]; }
+        const double sy = (double)dsum[4 * b] / dx, sx = (double)dsum[4 * b + 1] / dx;
+        const double s2 = (double)dsum[4 * b + 2] / ((double)dx * dx);
+        const double cy = cos(ty), cx = cos(tx);
+        const double ay = two_pi * dz * sy / (cy * cy), ax = two_pi * dz * sx / (cx * cx);
+        gz += -0.5 * two_pi * lambda * s2 + two_pi * (tan(tx) * sx + tan(ty) * sy);
+        if (tilt_mode == 2 && g_tilt) {
+            g_tilt[2 * b] = (accumulate ? g_tilt[2 * b] : 0.f) + (float)ay;
+            g_tilt[2 * b + 1] = (accumulate ? g_tilt[2 * b + 1] : 0.f) + (float)ax;
+        }
+        gty += ay; gtx += ax;
+    }
+    if (tilt_mode == 1 && g_tilt) {
+        g_tilt[0] = (accumulate ? g_tilt[0] : 0.f) + (float)gty;
+        g_tilt[1] = (accumulate ? g_tilt[1] : 0.f) + (float)gtx;
+    }
+    if (g_dz) g_dz[0] = (accumulate ? g_dz[0] : 0.f) + (float)gz;
+}
+
+// a14 (B9): bias-corrected Adam on a flat float array.  HBM-bound: streams theta, g, m, v.
+__global__ void __launch_bounds__(256) pty_adam_kernel(float* __restrict__ theta, const float* __restrict__ g,
+                                                       float* __restrict__ m, float* __restrict__ v, size_t n,
+                                                       float lr, float b1, float b2, float eps, float inv_bc1,
+                                                       float inv_bc2) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    const size_t n4 = n / 4;
+    float4* t4 = reinterpret_cast<float4*>(theta);
+    const float4* g4 = reinterpret_cast<const float4*>(g);
+    float4* m4 = reinterpret_cast<float4*>(m);
+    float4* v4 = reinterpret_cast<float4*>(v);
+    auto upd = [&](float& th, float gg, float& mm, float& vv) {
+        mm = b1 * mm + (1.f - b1) * gg;
+        vv = b2 * vv + (1.f - b2) * gg * gg;
+        th -= lr * (mm * inv_bc1) / (sqrtf(vv * inv_bc2) + eps);
+    };
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+        float4 th = t4[i], gg = __ldg(g4 + i), mm = m4[i], vv = v4[i];
+        upd(th.x, gg.x, mm.x, vv.x); upd(th.y, gg.y, mm.y, vv.y);
+        upd(th.z, gg.z, mm.z, vv.z); upd(th.w, gg.w, mm.w, vv.w);
+        t4[i] = th; m4[i] = mm; v4[i] = vv;
+    }
+    for (size_t i = n4 * 4 + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        float th = theta[i], mm = m[i], vv = v[i];
+        upd(th, g[i], mm, vv);
+        theta[i] = th; m[i] = mm; v[i] = vv;
+    }
+}
+
+// ============================================================================ host side
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Layout {
+    size_t probe_hat, prop, I, ws_psi, ws_Psi, ws_hat, GP_hat, dsum, scalars;
+    size_t g_object, g_probe, g_pos, g_tilt;               // PTY_FLAG_STEP / PTY_FLAG_HOST
+    size_t h_object, h_probe, h_pos, h_tilt, h_meas;       // PTY_FLAG_HOST staging
+    size_t total;
+};
+
+size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
+
+bool save_hat_of(const pty_dims& d) { return d.Nz > 1 && (d.tilt_mode != 0 || (d.flags & PTY_FLAG_SPECTRA)); }
+
+int validate_dims(const pty_dims* d, std::string& err) {
+    if (!d) { err = "dims is null"; return PTY_ERR_INVALID_ARG; }
+    if (d->Nz < 1 || d->M < 1 || d->Bmax < 1 || d->H < 1 || d->W < 1) { err = "non-positive dimension"; return PTY_ERR_INVALID_ARG; }
+    if (d->tilt_mode < 0 || d->tilt_mode > 2) { err = "tilt_mode must be 0, 1 or 2"; return PTY_ERR_INVALID_ARG; }
+    if (!(d->dx > 0.f) || !(d->lambda >= 0.f)) { err = "dx must be > 0 and lambda >= 0"; return PTY_ERR_INVALID_ARG; }
+    if (d->N != 64 && d->N != 128 && d->N != 256) { err = "N must be 64, 128 or 256"; return PTY_ERR_UNSUPPORTED; }
+    if (d->N > d->H || d->N > d->W) { err = "probe window larger than the object"; return PTY_ERR_UNSUPPORTED; }
+    return PTY_OK;
+}
+
+Layout make_layout(const pty_dims& d) {
+    Layout L{};
+    const size_t NN = (size_t)d.N * d.N, B = (size_t)d.Bmax, M = (size_t)d.M, Nz = (size_t)d.Nz;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+    L.probe_hat = take(M * NN * 8);
+    L.prop = take(2 * (size_t)d.N * 8);
+    L.I = take(B * NN * 4);
+    L.ws_psi = take(B * M * Nz * NN * 8);
+    L.ws_Psi = take(B * M * NN * 8);
+    L.ws_hat = take(save_hat_of(d) ? B * M * (Nz - 1) * NN * 8 : 0);
+    L.GP_hat = take(M * NN * 8);
+    L.dsum = take(B * 4 * 4);
+    L.scalars = take(256);
+    const bool grads = d.flags & (PTY_FLAG_STEP | PTY_FLAG_HOST);
+    const size_t obj = Nz * (size_t)d.H * d.W * 8;
+    L.g_object = take(grads ? obj : 0);
+    L.g_probe = take(grads ? M * NN * 8 : 0);
+    L.g_pos = take(grads ? B * 2 * 4 : 0);
+    L.g_tilt = take(grads ? B * 2 * 4 + 16 : 0);
+    const bool host = d.flags & PTY_FLAG_HOST;
+    L.h_object = take(host ? obj : 0);
+    L.h_probe = take(host ? M * NN * 8 : 0);
+    L.h_pos = take(host ? B * 2 * 4 : 0);
+    L.h_tilt = take(host ? B * 2 * 4 + 16 : 0);
+    L.h_meas = take(host ? B * NN * 4 : 0);
+    L.total = off;
+    return L;
+}
+
+}  // namespace
+
+struct pty_plan {
+    pty_dims d;
+    Layout L;
+    unsigned char* ws;
+    int device;
+    int num_sms;
+    std::string err;
+    cudaStream_t last_stream;
+    int64_t launches;
+    // state left by the last forward
+    bool fwd_valid;
+    const void *f_object, *f_probe, *f_positions, *f_tilt, *f_meas;
+    int32_t f_B;
+
+    // optional kernel timing (pty_profile)
+    bool profiling;
+    struct Timed { cudaEvent_t a, b; int which; };
+    std::vector<Timed> timed;
+
+    template <class T> T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
+    double* d_loss() const { return at<double>(L.scalars); }
+    int* d_flags() const { return at<int>(L.scalars + 64); }
+    float* d_gdz() const { return at<float>(L.scalars + 128); }
+};
+
+namespace {
+
+int fail(pty_plan* p, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (p) p->err = buf; else g_create_error = buf;
+    return code;
+}
+
+#define PTY_CUDA(p, call)                                                                     \
+    do {                                                                                      \
+        cudaError_t e_ = (call);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(p, PTY_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                                  \
+    } while (0)
+
+template <class K, class... Args>
+cudaError_t launch(pty_plan* p, K kernel, int grid, int block, size_t smem, int cluster, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    int na = 0;
+    if (cluster > 1) {
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = (unsigned)cluster;
+        attr[na].val.clusterDim.y = 1;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = na;
+    p->launches++;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
+template <class SH> cudaError_t set_smem_attrs() {
+    const int bytes = (int)ShapeInfo<SH>::smem_bytes;
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(pty_fwd_kernel<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e;
+    if ((e = cudaFuncSetAttribute(pty_bwd_kernel<SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e;
+    if ((e = cudaFuncSetAttribute(pty_fft2_kernel<SH, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e;
+    if ((e = cudaFuncSetAttribute(pty_fft2_kernel<SH, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))) return e;
+    return cudaSuccess;
+}
+
+template <class SH> cudaError_t launch_fft2(pty_plan* p, int dir, const float2* src, float2* dst, float scale, int acc, int items, cudaStream_t st) {
+    const size_t smem = ShapeInfo<SH>::smem_bytes;
+    if (dir < 0) return launch(p, pty_fft2_kernel<SH, -1>, items * SH::CL, SH::NT, smem, SH::CL, st, src, dst, scale, acc);
+    return launch(p, pty_fft2_kernel<SH, +1>, items * SH::CL, SH::NT, smem, SH::CL, st, src, dst, scale, acc);
+}
+// brackets one launch with events when pty_profile is on
+struct ScopedTimer {
+    pty_plan* p; cudaStream_t st; pty_plan::Timed t; bool on;
+    ScopedTimer(pty_plan* p_, int which, cudaStream_t st_) : p(p_), st(st_), on(false) {
+        if (!p->profiling || p->timed.size() >= 1024) return;
+        if (cudaEventCreate(&t.a) != cudaSuccess) return;
+        if (cudaEventCreate(&t.b) != cudaSuccess) { cudaEventDestroy(t.a); return; }
+        t.which = which; on = true;
+        cudaEventRecord(t.a, st);
+    }
+    ~ScopedTimer() {
+        if (!on) return;
+        cudaEventRecord(t.b, st);
+        p->timed.push_back(t);
+    }
+};
+
+template <class SH> cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
+    ScopedTimer tm(p, 0, st);
+    return launch(p, pty_fwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
+}
+template <class SH> cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
+    ScopedTimer tm(p, 1, st);
+    return launch(p, pty_bwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
+}
+
+#define PTY_DISPATCH_N(p, expr64, expr128, expr256)                     \
+    ((p)->d.N == 64 ? (expr64) : (p)->d.N == 128 ? (expr128) : (expr256))
+
+KArgs make_args(const pty_plan* p, const void* object, const float* positions, const float* tilt,
+                const float* meas, int32_t B) {
+    KArgs A{};
+    const pty_dims& d = p->d;
+    A.Nz = d.Nz; A.H = d.H; A.W = d.W; A.M = d.M; A.B = B;
+    A.tilt_mode = d.tilt_mode;
+    A.save_hat = save_hat_of(d) ? 1 : 0;
+    A.dz = d.dz; A.lambda = d.lambda; A.dx = d.dx;
+    A.object = static_cast<const float2*>(object);
+    A.probe_hat = p->at<float2>(p->L.probe_hat);
+    A.positions = positions;
+    A.tilt = tilt;
+    A.meas = meas;
+    A.prop_y = p->at<float2>(p->L.prop);
+    A.prop_x = p->at<float2>(p->L.prop) + d.N;
+    A.I = p->at<float>(p->L.I);
+    A.ws_psi = p->at<float2>(p->L.ws_psi);
+    A.ws_Psi = p->at<float2>(p->L.ws_Psi);
+    A.ws_hat = A.save_hat ? p->at<float2>(p->L.ws_hat) : nullptr;
+    A.GP_hat = p->at<float2>(p->L.GP_hat);
+    A.dsum = p->at<float>(p->L.dsum);
+    A.flags = p->d_flags();
+    return A;
+}
+
+int check_batch(pty_plan* p, const void* object, const void* probe, const float* positions, const float* tilt,
+                const float* meas, int32_t B) {
+    if (!p) return PTY_ERR_INVALID_ARG;
+    if (!object || !probe || !positions || !meas) return fail(p, PTY_ERR_INVALID_ARG, "null input pointer");
+    if (p->d.tilt_mode != 0 && !tilt) return fail(p, PTY_ERR_INVALID_ARG, "tilt_mode %d needs a tilt pointer", p->d.tilt_mode);
+    if (B < 0 || B > p->d.Bmax) return fail(p, PTY_ERR_INVALID_ARG, "B = %d outside [0, Bmax = %d]", B, p->d.Bmax);
+    return PTY_OK;
+}
+
+// a0 + a2..a6 for one minibatch
+int run_forward(pty_plan* p, const void* object, const void* probe, const float* positions, const float* tilt,
+                const float* meas, int32_t B, double* loss, float* loss_per_pos, float* intensity, cudaStream_t st) {
+    const pty_dims& d = p->d;
+    const size_t NN = (size_t)d.N * d.N;
+    p->last_stream = st;
+    p->fwd_valid = false;
+    PTY_CUDA(p, cudaMemsetAsync(loss, 0, sizeof(double), st));
+    if (B == 0) return PTY_OK;
+    KArgs A = make_args(p, object, positions, tilt, meas, B);
+    // a0: probe spectrum (unitary) and propagator factors
+    PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fft2<Shape<64>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
+                               launch_fft2<Shape<128>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
+                               launch_fft2<Shape<256>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st)));
+    if (d.tilt_mode != 2)
+        PTY_CUDA(p, launch(p, pty_prop_table_kernel, (d.N + 127) / 128, 128, 0, 1, st, (int)d.N, d.dz, d.lambda, d.dx,
+                           d.tilt_mode == 1 ? tilt : (const float*)nullptr, p->at<float2>(p->L.prop), p->at<float2>(p->L.prop) + d.N));
+    PTY_CUDA(p, cudaMemsetAsync(A.I, 0, (size_t)B * NN * sizeof(float), st));
+    PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fwd<Shape<64>>(p, A, st), launch_fwd<Shape<128>>(p, A, st), launch_fwd<Shape<256>>(p, A, st)));
+    PTY_CUDA(p, launch(p, pty_loss_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)NN, loss, loss_per_pos));
+    if (intensity)
+        PTY_CUDA(p, cudaMemcpyAsync(intensity, A.I, (size_t)B * NN * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    p->fwd_valid = true;
+    p->f_object = object; p->f_probe = probe; p->f_positions = positions; p->f_tilt = tilt; p->f_meas = meas;
+    p->f_B = B;
+    return PTY_OK;
+}
+
+// a7..a13 for one minibatch; needs the forward state
+int run_backward(pty_plan* p, const void* object, const float* positions, const float* tilt, const float* meas,
+                 int32_t B, void* g_object, void* g_probe, float* g_positions, float* g_tilt, float* g_dz,
+                 int accumulate, cudaStream_t st) {
+    const pty_dims& d = p->d;
+    const size_t NN = (size_t)d.N * d.N;
+    p->last_stream = st;
+    if (!accumulate) {
+        PTY_CUDA(p, cudaMemsetAsync(g_object, 0, (size_t)d.Nz * d.H * d.W * sizeof(float2), st));
+        if (g_positions && B) PTY_CUDA(p, cudaMemsetAsync(g_positions, 0, (size_t)B * 2 * sizeof(float), st));
+    }
+    KArgs A = make_args(p, object, positions, tilt, meas, B);
+    A.g_object = static_cast<float2*>(g_object);
+    A.g_pos = g_positions;
+    const bool want_probe = g_probe != nullptr;
+    PTY_CUDA(p, cudaMemsetAsync(A.GP_hat, 0, (size_t)d.M * NN * sizeof(float2), st));
+    if (A.save_hat && B) PTY_CUDA(p, cudaMemsetAsync(A.dsum, 0, (size_t)B * 4 * sizeof(float), st));
+    if (B)
+        PTY_CUDA(p, PTY_DISPATCH_N(p, launch_bwd<Shape<64>>(p, A, st), launch_bwd<Shape<128>>(p, A, st), launch_bwd<Shape<256>>(p, A, st)));
+    if (want_probe)
+        PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fft2<Shape<64>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st),
+                                   launch_fft2<Shape<128>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st),
+                                   launch_fft2<Shape<256>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st)));
+    const bool want_tilt = g_tilt && d.tilt_mode != 0;
+    if (want_tilt || g_dz) {
+        if (A.save_hat) {
+            PTY_CUDA(p, launch(p, pty_tilt_finalize_kernel, 1, 32, 0, 1, st, (const float*)A.dsum, tilt, (int)B, (int)d.tilt_mode,
+                               d.dz, d.lambda, d.dx, want_tilt ? g_tilt : (float*)nullptr, g_dz, accumulate));
+        } else if (!accumulate) {   // Nz == 1: no propagation, so both gradients are exactly zero
+            if (want_tilt) PTY_CUDA(p, cudaMemsetAsync(g_tilt, 0, (d.tilt_mode == 2 ? (size_t)B * 2 : 2) * sizeof(float), st));
+            if (g_dz) PTY_CUDA(p, cudaMemsetAsync(g_dz, 0, sizeof(float), st));
+        }
+    }
+    return PTY_OK;
+}
+
+int adam_launch(pty_plan* p, float* theta, const float* g, float* m, float* v, size_t n, float lr, float b1, float b2,
+                float eps, int32_t t, cudaStream_t st) {
+    if (n == 0 || lr == 0.f) return PTY_OK;
+    if (!theta || !g || !m || !v) return fail(p, PTY_ERR_INVALID_ARG, "adam: null pointer");
+    if (t < 1) return fail(p, PTY_ERR_INVALID_ARG, "adam: step number t must be >= 1");
+    const float inv_bc1 = (float)(1.0 / (1.0 - pow((double)b1, (double)t)));
+    const float inv_bc2 = (float)(1.0 / (1.0 - pow((double)b2, (double)t)));
+    size_t blocks = (n / 4 + 255) / 256;
+    const size_t cap = (size_t)p->num_sms * 16;
+    if (blocks > cap) blocks = cap;
+    if (blocks == 0) blocks = 1;
+    PTY_CUDA(p, launch(p, pty_adam_kernel, (int)blocks, 256, 0, 1, st, theta, g, m, v, n, lr, b1, b2, eps, inv_bc1, inv_bc2));
+    return PTY_OK;
+}
+
+}  // namespace
+
+// ============================================================================ C ABI
+extern "C" {
+
+const char* pty_version(void) { return "pty-b200 0.1 (sm_100a)"; }
+
+int pty_workspace_bytes(const pty_dims* dims, size_t* out_bytes) {
+    std::string err;
+    int rc = validate_dims(dims, err);
+    if (rc != PTY_OK) { g_create_error = err; return rc; }
+    if (!out_bytes) { g_create_error = "out_bytes is null"; return PTY_ERR_INVALID_ARG; }
+    *out_bytes = make_layout(*dims).total;
+    return PTY_OK;
+}
+
+int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_t workspace_bytes, int device) {
+    if (!out_plan) { g_create_error = "out_plan is null"; return PTY_ERR_INVALID_ARG; }
+    *out_plan = nullptr;
+    std::string err;
+    int rc = validate_dims(dims, err);
+    if (rc != PTY_OK) { g_create_error = err; return rc; }
+    Layout L = make_layout(*dims);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255) != 0 || workspace_bytes < L.total)
+        return fail(nullptr, PTY_ERR_WORKSPACE, "workspace null, not 256-byte aligned or smaller than %zu bytes", L.total);
+    pty_plan* p = new (std::nothrow) pty_plan();
+    if (!p) return fail(nullptr, PTY_ERR_INVALID_ARG, "out of host memory");
+    p->d = *dims; p->L = L; p->ws = static_cast<unsigned char*>(workspace); p->device = device;
+    p->last_stream = nullptr; p->launches = 0; p->fwd_valid = false; p->profiling = false;
+    cudaError_t e = cudaSetDevice(device);
+    cudaDeviceProp prop{};
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e == cudaSuccess && prop.major < 10) {
+        delete p;
+        return fail(nullptr, PTY_ERR_UNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor);
+    }
+    if (e == cudaSuccess) e = PTY_DISPATCH_N(p, set_smem_attrs<Shape<64>>(), set_smem_attrs<Shape<128>>(), set_smem_attrs<Shape<256>>());
+    if (e == cudaSuccess) e = cudaMemset(p->ws + L.scalars, 0, 256);
+    if (e != cudaSuccess) {
+        delete p;
+        return fail(nullptr, PTY_ERR_CUDA, "pty_create: %s", cudaGetErrorString(e));
+    }
+    p->num_sms = prop.multiProcessorCount;
+    *out_plan = p;
+    return PTY_OK;
+}
+
+static void drop_timers(pty_plan* p) {
+    for (auto& t : p->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
+    p->timed.clear();
+}
+
+int pty_destroy(pty_plan* plan) {
+    if (plan) drop_timers(plan);
+    delete plan;
+    return PTY_OK;
+}
+
+int pty_profile(pty_plan* plan, int32_t enable) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    plan->profiling = enable != 0;
+    if (!enable) drop_timers(plan);
+    return PTY_OK;
+}
+
+int pty_profile_read(pty_plan* plan, float* fwd_ms, int32_t* fwd_launches, float* bwd_ms, int32_t* bwd_launches) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    PTY_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
+    float ms[2] = {0.f, 0.f};
+    int32_t n[2] = {0, 0};
+    for (auto& t : plan->timed) {
+        float e = 0.f;
+        PTY_CUDA(plan, cudaEventElapsedTime(&e, t.a, t.b));
+        ms[t.which] += e;
+        n[t.which]++;
+    }
+    drop_timers(plan);
+    if (fwd_ms) *fwd_ms = ms[0];
+    if (fwd_launches) *fwd_launches = n[0];
+    if (bwd_ms) *bwd_ms = ms[1];
+    if (bwd_launches) *bwd_launches = n[1];
+    return PTY_OK;
+}
+
+int pty_forward_loss(pty_plan* plan, const void* object, const void* probe, const float* positions, const float* tilt,
+                     const float* meas_amp, int32_t B, double* loss, float* loss_per_pos, float* intensity, void* stream) {
+    int rc = check_batch(plan, object, probe, positions, tilt, meas_amp, B);
+    if (rc != PTY_OK) return rc;
+    if (!loss) return fail(plan, PTY_ERR_INVALID_ARG, "loss is null");
+    return run_forward(plan, object, probe, positions, tilt, meas_amp, B, loss, loss_per_pos, intensity,
+                       static_cast<cudaStream_t>(stream));
+}
+
+int pty_backward(pty_plan* plan, const void* object, const void* probe, const float* positions, const float* tilt,
+                 const float* meas_amp, int32_t B, void* g_object, void* g_probe, float* g_positions, float* g_tilt,
+                 float* g_dz, int32_t flags, void* stream) {
+    int rc = check_batch(plan, object, probe, positions, tilt, meas_amp, B);
+    if (rc != PTY_OK) return rc;
+    if (!g_object) return fail(plan, PTY_ERR_INVALID_ARG, "g_object is null");
+    if (g_dz && plan->d.Nz > 1 && !save_hat_of(plan->d))
+        return fail(plan, PTY_ERR_INVALID_ARG, "g_dz needs tilt_mode != 0 or PTY_FLAG_SPECTRA");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool reuse = !(flags & PTY_BWD_RECOMPUTE) && plan->fwd_valid && plan->f_object == object &&
+                       plan->f_probe == probe && plan->f_positions == positions && plan->f_tilt == tilt &&
+                       plan->f_meas == meas_amp && plan->f_B == B && plan->last_stream == st;
+    if (!reuse) {
+        rc = run_forward(plan, object, probe, positions, tilt, meas_amp, B, plan->d_loss(), nullptr, nullptr, st);
+        if (rc != PTY_OK) return rc;
+    }
+    return run_backward(plan, object, positions, tilt, meas_amp, B, g_object, g_probe, g_positions, g_tilt, g_dz,
+                        (flags & PTY_BWD_ACCUMULATE) ? 1 : 0, st);
+}
+
+int pty_adam_update(pty_plan* plan, float* theta, const float* grad, float* m, float* v, size_t n, float lr,
+                    float beta1, float beta2, float eps, int32_t t, void* stream) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    plan->last_stream = static_cast<cudaStream_t>(stream);
+    return adam_launch(plan, theta, grad, m, v, n, lr, beta1, beta2, eps, t, static_cast<cudaStream_t>(stream));
+}
+
+int pty_step(pty_plan* plan, void* object, void* probe, float* positions, float* tilt, const float* meas_amp,
+             int32_t B, const pty_adam* hp, const pty_adam_state* s, double* loss, void* stream) {
+    int rc = check_batch(plan, object, probe, positions, tilt, meas_amp, B);
+    if (rc != PTY_OK) return rc;
+    if (!hp || !s || !loss) return fail(plan, PTY_ERR_INVALID_ARG, "hp, st or loss is null");
+    if (!(plan->d.flags & PTY_FLAG_STEP)) return fail(plan, PTY_ERR_INVALID_ARG, "plan was created without PTY_FLAG_STEP");
+    const pty_dims& d = plan->d;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    float2* g_object = plan->at<float2>(plan->L.g_object);
+    float2* g_probe = plan->at<float2>(plan->L.g_probe);
+    float* g_pos = plan->at<float>(plan->L.g_pos);
+    float* g_tilt = plan->at<float>(plan->L.g_tilt);
+    rc = run_forward(plan, object, probe, positions, tilt, meas_amp, B, loss, nullptr, nullptr, st);
+    if (rc != PTY_OK) return rc;
+    const bool tilt_on = d.tilt_mode != 0 && hp->lr_tilt != 0.f;
+    rc = run_backward(plan, object, positions, tilt, meas_amp, B, g_object, hp->lr_probe != 0.f ? g_probe : nullptr,
+                      hp->lr_positions != 0.f ? g_pos : nullptr, tilt_on ? g_tilt : nullptr, nullptr, 0, st);
+    if (rc != PTY_OK) return rc;
+    plan->fwd_valid = false;   // the parameters change below
+    const size_t NN = (size_t)d.N * d.N;
+    if ((rc = adam_launch(plan, (float*)object, (const float*)g_object, s->m_object, s->v_object,
+                          (size_t)d.Nz * d.H * d.W * 2, hp->lr_object, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    if ((rc = adam_launch(plan, (float*)probe, (const float*)g_probe, s->m_probe, s->v_probe, (size_t)d.M * NN * 2,
+                          hp->lr_probe, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    if ((rc = adam_launch(plan, positions, g_pos, s->m_positions, s->v_positions, (size_t)B * 2, hp->lr_positions,
+                          hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    if (tilt_on)
+        if ((rc = adam_launch(plan, tilt, g_tilt, s->m_tilt, s->v_tilt, d.tilt_mode == 2 ? (size_t)B * 2 : 2, hp->lr_tilt,
+                              hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    return PTY_OK;
+}
+
+int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, const float* h_positions,
+                  const float* h_tilt, const float* h_meas_amp, int32_t B, double* h_loss, void* h_g_object,
+                  void* h_g_probe, float* h_g_positions, float* h_g_tilt, void* stream) {
+    int rc = check_batch(plan, h_object, h_probe, h_positions, h_tilt, h_meas_amp, B);
+    if (rc != PTY_OK) return rc;
+    if (!(plan->d.flags & PTY_FLAG_HOST)) return fail(plan, PTY_ERR_INVALID_ARG, "plan was created without PTY_FLAG_HOST");
+    const pty_dims& d = plan->d;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t NN = (size_t)d.N * d.N, obj_bytes = (size_t)d.Nz * d.H * d.W * 8, probe_bytes = (size_t)d.M * NN * 8;
+    const size_t tilt_n = d.tilt_mode == 2 ? (size_t)B * 2 : 2;
+    float2* dobj = plan->at<float2>(plan->L.h_object);
+    float2* dprobe = plan->at<float2>(plan->L.h_probe);
+    float* dpos = plan->at<float>(plan->L.h_pos);
+    float* dtilt = d.tilt_mode ? plan->at<float>(plan->L.h_tilt) : nullptr;
+    float* dmeas = plan->at<float>(plan->L.h_meas);
+    PTY_CUDA(plan, cudaMemcpyAsync(dobj, h_object, obj_bytes, cudaMemcpyHostToDevice, st));
+    PTY_CUDA(plan, cudaMemcpyAsync(dprobe, h_probe, probe_bytes, cudaMemcpyHostToDevice, st));
+    if (B) PTY_CUDA(plan, cudaMemcpyAsync(dpos, h_positions, (size_t)B * 8, cudaMemcpyHostToDevice, st));
+    if (dtilt) PTY_CUDA(plan, cudaMemcpyAsync(dtilt, h_tilt, tilt_n * 4, cudaMemcpyHostToDevice, st));
+    if (B) PTY_CUDA(plan, cudaMemcpyAsync(dmeas, h_meas_amp, (size_t)B * NN * 4, cudaMemcpyHostToDevice, st));
+    rc = run_forward(plan, dobj, dprobe, dpos, dtilt, dmeas, B, plan->d_loss(), nullptr, nullptr, st);
+    if (rc != PTY_OK) return rc;
+    float2* g_object = plan->at<float2>(plan->L.g_object);
+    float2* g_probe = plan->at<float2>(plan->L.g_probe);
+    float* g_pos = plan->at<float>(plan->L.g_pos);
+    float* g_tilt = plan->at<float>(plan->L.g_tilt);
+    rc = run_backward(plan, dobj, dpos, dtilt, dmeas, B, g_object, h_g_probe ? g_probe : nullptr,
+                      h_g_positions ? g_pos : nullptr, (h_g_tilt && dtilt) ? g_tilt : nullptr, nullptr, 0, st);
+    if (rc != PTY_OK) return rc;
+    if (h_loss) PTY_CUDA(plan, cudaMemcpyAsync(h_loss, plan->d_loss(), 8, cudaMemcpyDeviceToHost, st));
+    if (h_g_object) PTY_CUDA(plan, cudaMemcpyAsync(h_g_object, g_object, obj_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_g_probe) PTY_CUDA(plan, cudaMemcpyAsync(h_g_probe, g_probe, probe_bytes, cudaMemcpyDeviceToHost, st));
+    if (h_g_positions && B) PTY_CUDA(plan, cudaMemcpyAsync(h_g_positions, g_pos, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    if (h_g_tilt && dtilt) PTY_CUDA(plan, cudaMemcpyAsync(h_g_tilt, g_tilt, tilt_n * 4, cudaMemcpyDeviceToHost, st));
+    PTY_CUDA(plan, cudaStreamSynchronize(st));
+    return PTY_OK;
+}
+
+int pty_status(pty_plan* plan, int32_t* device_flags) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    PTY_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
+    int flags = 0;
+    PTY_CUDA(plan, cudaMemcpy(&flags, plan->d_flags(), sizeof(int), cudaMemcpyDeviceToHost));
+    PTY_CUDA(plan, cudaMemset(plan->d_flags(), 0, sizeof(int)));
+    if (device_flags) *device_flags = flags;
+    PTY_CUDA(plan, cudaGetLastError());
+    if (flags & 1) return fail(plan, PTY_ERR_BOUNDS, "a scan position's crop left the object and was clamped");
+    return PTY_OK;
+}
+
+int64_t pty_launch_count(const pty_plan* plan) { return plan ? plan->launches : 0; }
+
+const char* pty_last_error(const pty_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"
