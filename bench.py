@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the multislice-ptychography hot path on B200.
+
+A "step" is one pass of the whole hot path over one minibatch of synthetic input: pty_forward_loss
+followed by pty_backward (object, probe and position gradients; tilt too on config 5).  Metric
+(BASELINE.json): diffraction patterns/s per forward+gradient pass, plus the fraction of the
+FFT-FLOP roofline of the dominant kernel.  Default workload: config 4 (128^2 detector, 12 probe
+modes, 6 slices, 1088^2 object, 128x128 scan), minibatch 1024 -- the headline roofline config.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--batch B] [--impl reference]
+
+N > 1 is launched by torchrun (one rank per GPU); each rank runs its own minibatches (weak scaling)
+and the object/probe gradients are all-reduced over NCCL inside the timed step (the one real
+exchange of data-parallel ptychography).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "patterns_per_s_forward_gradient"
+UNIT = "patterns/s"
+FP32_LANES_PER_SM = 128      # B200: 4 SMSP x 32 FP32 lanes; 2 flops per FMA
+
+
+def fft_flops_per_pattern(cfg, with_tilt):
+    """Nominal 2-D FFT flops: 10 N^2 log2 N each; 4 Nz per (position, mode)."""
+    n_fft = 4 * cfg.Nz * cfg.M
+    return n_fft * 10.0 * cfg.N * cfg.N * math.log2(cfg.N)
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons of one GPU while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.lines = []
+        self.proc = None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------ reference arm
+def run_reference(args, cfg, B):
+    """--impl reference: the float64 oracle as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    from paper_2505_07814_b200 import synth
+    cores = len(os.sched_getaffinity(0))
+    geom = oracle.Geometry(cfg.dz, cfg.lam, cfg.dx)
+    tr, ev = synth.truth(cfg), synth.eval_point(cfg, "A")
+    n = max(4, min(B, 2 * cores))
+    idx = synth.minibatch(cfg, 0, B)[:n]
+    tilt_t = tr["tilt"] if cfg.tilt_mode else None
+    tilt_e = ev["tilt"] if cfg.tilt_mode else None
+    meas = synth.poisson_amplitudes(cfg, oracle.intensity_batch(tr["object"], tr["probe"], tr["positions"][idx],
+                                                                tilt_t, geom), idx)
+    pos = np.ascontiguousarray(ev["positions"][idx])
+    run = lambda: oracle.grad_batch(ev["object"], ev["probe"], pos, tilt_e, meas, geom, workers=cores)
+    for _ in range(args.warmup):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run()
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = f"{n} positions of minibatch 0 of config {cfg.c} per step (of B={B}), float64 numpy, {cores} worker processes"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, B, extra={"sample": sample}),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def workload_config(cfg, B, extra=None):
+    d = {"workload": f"c{cfg.c}: {cfg.N}x{cfg.N} detector, {cfg.M} probe modes, {cfg.Nz} slices, "
+                     f"{cfg.H}x{cfg.W} object, {cfg.ns}x{cfg.ns} scan, minibatch {B}",
+         "config_index": cfg.c - 1, "N": cfg.N, "M": cfg.M, "Nz": cfg.Nz, "object": [cfg.Nz, cfg.H, cfg.W],
+         "minibatch": B, "n_positions": cfg.n_positions, "dose": cfg.dose, "tilt_mode": cfg.tilt_mode,
+         "gradients": "object,probe,positions" + (",tilt" if cfg.tilt_mode else ""),
+         "cache": "inputs larger than L2: every step reads a different minibatch and streams its saved waves "
+                  "through HBM (>= several GB per step at the default size)"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ------------------------------------------------------------------------------ our arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--batch", type=int, default=None)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+
+    from paper_2505_07814_b200 import synth
+    cfg = synth.get_config(args.config)
+    B = args.batch or cfg.B
+    if args.impl == "reference":
+        run_reference(args, cfg, B)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2505_07814_b200 import build
+    build.build()
+    from paper_2505_07814_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    # ---- synthetic dataset: truth -> measurements (library forward + Poisson), evaluation point A
+    tr, ev = synth.truth(cfg), synth.eval_point(cfg, "A")
+    nb_total = max(1, cfg.n_positions // B)
+    n_used = min(nb_total, args.steps + args.warmup)
+    my_batches = [(rank + world * j) % nb_total for j in range(n_used)]
+    want_e2e = not args.no_e2e
+    plan = binding.plan_for(cfg, Bmax=B, flags=binding.PTY_FLAG_HOST if want_e2e else 0, device=local)
+    to = lambda x: None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(dev)
+    obj_t, probe_t = to(tr["object"]), to(tr["probe"])
+    tilt_t = to(tr["tilt"]) if cfg.tilt_mode else None
+    obj, probe = to(ev["object"]), to(ev["probe"])
+    tilt = to(ev["tilt"]) if cfg.tilt_mode else None
+    pos_batches, meas_batches = [], []
+    inten = torch.empty(B, cfg.N, cfg.N, dtype=torch.float32, device=dev)
+    gen = torch.Generator(device=dev)
+    for j in my_batches:
+        idx = synth.minibatch(cfg, j, B)
+        gen.manual_seed(1000 * cfg.c + 3 + 7919 * j)
+        zeros = torch.zeros(B, cfg.N, cfg.N, dtype=torch.float32, device=dev)
+        plan.forward_loss(obj_t, probe_t, to(tr["positions"][idx]), tilt_t, zeros, intensity=inten)
+        meas_batches.append(torch.sqrt(torch.poisson(inten.clamp_min(0), generator=gen)))
+        pos_batches.append(to(ev["positions"][idx]))
+    del obj_t, probe_t, inten, zeros
+
+    g_obj, g_probe = torch.zeros_like(obj), torch.zeros_like(probe)
+    g_pos = torch.zeros(B, 2, device=dev)
+    g_tilt = torch.zeros(2, device=dev) if cfg.tilt_mode else None
+    loss = torch.zeros(1, dtype=torch.float64, device=dev)
+
+    def step(i):
+        j = i % n_used
+        plan.forward_loss(obj, probe, pos_batches[j], tilt, meas_batches[j], loss)
+        plan.backward(obj, probe, pos_batches[j], tilt, meas_batches[j], g_obj, g_probe, g_pos, g_tilt)
+        if world > 1:
+            dist.all_reduce(torch.view_as_real(g_obj))
+            dist.all_reduce(torch.view_as_real(g_probe))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    rc, _ = plan.status()
+    if rc != 0:
+        raise SystemExit(f"pty_status = {rc}: {plan.last_error()}")
+    plan.profile(True)
+    l0 = plan.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        barrier()
+        e0.record()
+        for i in range(args.steps):
+            step(args.warmup + i)
+        e1.record()
+        barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = plan.launch_count() - l0
+    prof = plan.profile_read()
+    plan.profile(False)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = t.item()
+    value = world * B * args.steps / (ms_total * 1e-3)
+    final_loss = loss.item()
+
+    # ---- end to end through the host-buffer entry point (H2D of every input, D2H of loss + gradients)
+    e2e = None
+    if want_e2e:
+        pin = lambda t: t.cpu().pin_memory()
+        h_obj, h_probe = pin(obj), pin(probe)
+        h_tilt = pin(tilt) if tilt is not None else None
+        h_pos = [pin(p) for p in pos_batches[:3]]
+        h_meas = [pin(m) for m in meas_batches[:3]]
+        h_loss = torch.zeros(1, dtype=torch.float64).pin_memory()
+        h_go, h_gp = torch.zeros_like(h_obj).pin_memory(), torch.zeros_like(h_probe).pin_memory()
+        h_gq = torch.zeros(B, 2).pin_memory()
+        h_gt = torch.zeros(2).pin_memory() if tilt is not None else None
+        k_e2e = max(2, min(args.steps, 5))
+        run = lambda i: plan.grad_host(h_obj, h_probe, h_pos[i % len(h_pos)], h_tilt, h_meas[i % len(h_meas)], h_loss,
+                                       h_go, h_gp, h_gq, h_gt)
+        run(0)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(k_e2e):
+            run(i + 1)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = t.item()
+        h2d = h_obj.numel() * 8 + h_probe.numel() * 8 + B * 8 + B * cfg.N * cfg.N * 4 + (8 if tilt is not None else 0)
+        d2h = 8 + h_go.numel() * 8 + h_gp.numel() * 8 + B * 8 + (8 if tilt is not None else 0)
+        e2e = {"value": world * B * k_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": k_e2e, "api": "pty_grad_host (pinned host buffers)",
+               "loss": float(h_loss.item())}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (FP32 ALU bound)
+    peaks, peaks_src = load_peaks()
+    clocks = clk.summary()
+    sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0)
+    n_sms = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_tf = n_sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    flops_launch = 0.5 * fft_flops_per_pattern(cfg, cfg.tilt_mode) * B     # each kernel does 2 Nz M FFTs / pattern
+    kern = {}
+    for name in ("fwd", "bwd"):
+        ms, n = prof[name]
+        if n:
+            kern[name] = {"avg_ms": ms / n, "launches": n, "tflops": flops_launch / (ms / n * 1e-3) / 1e12}
+    dom = max(kern, key=lambda k: kern[k]["avg_ms"]) if kern else None
+    roofline = None
+    if dom:
+        a = kern[dom]["tflops"]
+        roofline = {"bound": "alu", "kernel": f"pty_{dom}_kernel<Shape<{cfg.N}>>", "achieved": a, "peak": peak_tf,
+                    "unit": "TFLOP/s", "frac": a / peak_tf, "traffic": None,
+                    "peak_source": f"{n_sms} SMs x 128 FP32 lanes x 2 flop x clocks.max.sm {sm_max:.0f} MHz "
+                                   "(nominal FP32 FMA peak; HBM is not the bound, DESIGN.md)",
+                    "algorithmic_flops_per_launch": flops_launch, "avg_launch_ms": kern[dom]["avg_ms"],
+                    "kernels": kern,
+                    "whole_step_frac_of_fft_roofline": value * fft_flops_per_pattern(cfg, 0) / world / 1e12 / peak_tf,
+                    "hbm_peak_gbs": peaks.get("hbm_gbs"), "peaks": peaks_src}
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            try:
+                roofline["traffic"] = json.load(open(tp)).get(f"c{cfg.c}_B{B}_{dom}")
+            except Exception:
+                pass
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, B),
+           "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "loss": final_loss}
+    if e2e:
+        out["e2e"] = e2e
+
+    # ---- the oracle timed on this box's host cores (a reported baseline, not the target)
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        cores = len(os.sched_getaffinity(0))
+        geom = oracle.Geometry(cfg.dz, cfg.lam, cfg.dx)
+        per_pattern_s = {1: 0.002, 2: 0.03, 3: 0.07, 4: 0.14, 5: 1.4}[cfg.c]
+        n = int(max(4, min(B, round(20.0 * cores / per_pattern_s / cores / 8) * 1)))   # ~ 20 s of CPU work / 8
+        n = max(4, min(B, max(cores, n)))
+        idx = synth.minibatch(cfg, 0, B)[:n]
+        tilt_tr = tr["tilt"] if cfg.tilt_mode else None
+        tilt_ev = ev["tilt"] if cfg.tilt_mode else None
+        meas = synth.poisson_amplitudes(cfg, oracle.intensity_batch(tr["object"], tr["probe"], tr["positions"][idx],
+                                                                    tilt_tr, geom), idx)
+        pos = np.ascontiguousarray(ev["positions"][idx])
+        t0 = time.perf_counter()
+        ref = oracle.grad_batch(ev["object"], ev["probe"], pos, tilt_ev, meas, geom, workers=cores)
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": f"{n} positions of minibatch 0 (of B={B}), forward + all gradients, float64 "
+                                         f"numpy, {cores} worker processes, {dt:.1f} s"}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -139,8 +139,8 @@ __global__ void pty_tilt_finalize_kernel(const float* dsum, const float* tilt, i
 // a14 (B9): bias-corrected Adam on a flat float array.  HBM-bound: streams theta, g, m, v.
 __global__ void __launch_bounds__(256) pty_adam_kernel(float* __restrict__ theta, const float* __restrict__ g,
                                                        float* __restrict__ m, float* __restrict__ v, size_t n,
-                                                       float lr, float b1, float b2, float eps, float inv_bc1,
-                                                       float inv_bc2) {
+                                                       float lr, float b1, float b2, float omb1, float omb2,
+                                                       float eps, float inv_bc1, float inv_bc2) {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     const size_t n4 = n / 4;
     float4* t4 = reinterpret_cast<float4*>(theta);
@@ -148,8 +148,8 @@ __global__ void __launch_bounds__(256) pty_adam_kernel(float* __restrict__ theta
     float4* m4 = reinterpret_cast<float4*>(m);
     float4* v4 = reinterpret_cast<float4*>(v);
     auto upd = [&](float& th, float gg, float& mm, float& vv) {
-        mm = b1 * mm + (1.f - b1) * gg;
-        vv = b2 * vv + (1.f - b2) * gg * gg;
+        mm = b1 * mm + omb1 * gg;
+        vv = b2 * vv + omb2 * gg * gg;
         th -= lr * (mm * inv_bc1) / (sqrtf(vv * inv_bc2) + eps);
     };
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
@@ -362,7 +362,7 @@ KArgs make_args(const pty_plan* p, const void* object, const float* positions, c
 int check_batch(pty_plan* p, const void* object, const void* probe, const float* positions, const float* tilt,
                 const float* meas, int32_t B) {
     if (!p) return PTY_ERR_INVALID_ARG;
-    if (!object || !probe || !positions || !meas) return fail(p, PTY_ERR_INVALID_ARG, "null input pointer");
+    if (!object || !probe || (B > 0 && (!positions || !meas))) return fail(p, PTY_ERR_INVALID_ARG, "null input pointer");
     if (p->d.tilt_mode != 0 && !tilt) return fail(p, PTY_ERR_INVALID_ARG, "tilt_mode %d needs a tilt pointer", p->d.tilt_mode);
     if (B < 0 || B > p->d.Bmax) return fail(p, PTY_ERR_INVALID_ARG, "B = %d outside [0, Bmax = %d]", B, p->d.Bmax);
     return PTY_OK;
@@ -443,7 +443,9 @@ int adam_launch(pty_plan* p, float* theta, const float* g, float* m, float* v, s
     const size_t cap = (size_t)p->num_sms * 16;
     if (blocks > cap) blocks = cap;
     if (blocks == 0) blocks = 1;
-    PTY_CUDA(p, launch(p, pty_adam_kernel, (int)blocks, 256, 0, 1, st, theta, g, m, v, n, lr, b1, b2, eps, inv_bc1, inv_bc2));
+    const float omb1 = (float)(1.0 - (double)b1), omb2 = (float)(1.0 - (double)b2);   // 1 - beta rounded once
+    PTY_CUDA(p, launch(p, pty_adam_kernel, (int)blocks, 256, 0, 1, st, theta, g, m, v, n, lr, b1, b2, omb1, omb2, eps,
+                       inv_bc1, inv_bc2));
     return PTY_OK;
 }
 

@@ -47,9 +47,20 @@ def make_case(c, which, indices, tilt_mode=None):
     if tm == 2:
         rng = np.random.default_rng(1000 * c + 77)
         tilt = (ev["tilt"][None, :] + rng.normal(0, 2e-4, (len(indices), 2))).astype(np.float32)
-    return {"cfg": cfg, "object": ev["object"], "probe": ev["probe"],
+    case = {"cfg": cfg, "object": ev["object"], "probe": ev["probe"],
             "positions": np.ascontiguousarray(ev["positions"][indices]), "tilt": tilt, "tilt_mode": tm,
             "meas": meas, "indices": indices}
+    if which == "B":
+        # DESIGN.md reading R26: at the exact-vacuum start the model's dark field is float32 rounding
+        # noise (I ~ 1e-14 of the peak), and d/dPsi (|Psi| - a)^2 = 2 (1 - a/|Psi|) Psi has a phase set
+        # by that noise wherever counts a > 0 were measured: the gradient is ill-conditioned there in
+        # any float32 arithmetic.  Gradients at point B are therefore compared with the counts of those
+        # pixels (model intensity below 1e-9 of the pattern's peak, per the ORACLE) set to zero; the
+        # loss and the intensities are compared on the full measurements.
+        I_B = oracle.intensity_batch(case["object"], case["probe"], case["positions"], tilt, geom_of(cfg))
+        dark = I_B < 1e-9 * I_B.max(axis=(1, 2), keepdims=True)
+        case["meas_masked"] = np.where(dark, 0.0, meas).astype(np.float32)
+    return case
 
 
 def oracle_grad(case, workers=None):

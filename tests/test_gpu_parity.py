@@ -61,20 +61,30 @@ def run_gpu(pty, case, want_dz=False, flags=0, plan=None, bwd_flags=0, outputs=N
     return res
 
 
-def check_against_oracle(res, ref, case, check_intensity=True):
+def check_against_oracle(res, ref, case, scale_ref=None):
+    """Loss within 1e-4, every gradient within 1e-3 relative L2.  `scale_ref` (evaluation point B
+    only, R26): position / tilt / dz gradients vanish analytically for a vacuum object, so their
+    error is measured against the same gradient's norm at evaluation point A when that is larger."""
     cfg = case["cfg"]
     assert res["status"] == 0
     assert abs(res["loss"][0] - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"]), (res["loss"][0], ref["loss"])
     np.testing.assert_allclose(res["loss_per_pos"], ref["loss_per_pos"], rtol=LOSS_RTOL)
-    errs = {"g_object": rel_l2(res["g_object"], ref["g_object"]),
-            "g_probe": rel_l2(res["g_probe"], ref["g_probe"]),
-            "g_positions": rel_l2(res["g_positions"], ref["g_positions"])}
+
+    def err(x, r, key=None, reduce=lambda a: a):
+        den = np.linalg.norm(np.ravel(reduce(r)))
+        if scale_ref is not None and key is not None:
+            den = max(den, np.linalg.norm(np.ravel(reduce(scale_ref[key]))))
+        return float(np.linalg.norm(np.ravel(x - reduce(r))) / max(den, 1e-300))
+
+    errs = {"g_object": err(res["g_object"], ref["g_object"]),
+            "g_probe": err(res["g_probe"], ref["g_probe"]),
+            "g_positions": err(res["g_positions"], ref["g_positions"], "g_positions")}
     if case["tilt_mode"] == 2:
-        errs["g_tilt"] = rel_l2(res["g_tilt"], ref["g_tilt"])
+        errs["g_tilt"] = err(res["g_tilt"], ref["g_tilt"], "g_tilt")
     elif case["tilt_mode"] == 1:
-        errs["g_tilt"] = rel_l2(res["g_tilt"], ref["g_tilt"].sum(0))
+        errs["g_tilt"] = err(res["g_tilt"], ref["g_tilt"], "g_tilt", reduce=lambda a: a.sum(0))
     if res["g_dz"] is not None and cfg.Nz > 1:
-        errs["g_dz"] = abs(res["g_dz"][0] - ref["g_dz"]) / abs(ref["g_dz"])
+        errs["g_dz"] = err(res["g_dz"][0], np.float64(ref["g_dz"]), "g_dz")
     bad = {k: v for k, v in errs.items() if not v <= GRAD_RTOL}
     assert not bad, f"gradients outside {GRAD_RTOL}: {bad} (all: {errs})"
     return errs
@@ -91,6 +101,16 @@ def test_parity_all_configs(pty, c, which, B):
     cfg = synth.get_config(c)
     idx = synth.minibatch(cfg, 0, cfg.B)[:B]
     case = make_case(c, which, idx)
+    if which == "B":      # ill-conditioned dark-field pixels: loss on the full data, gradients masked (R26)
+        full = run_gpu(pty, case)
+        L, lb, _ = oracle.forward_loss_batch(case["object"], case["probe"], case["positions"], case["tilt"],
+                                             case["meas"], geom_of(cfg))
+        assert abs(full["loss"][0] - L) <= LOSS_RTOL * L
+        np.testing.assert_allclose(full["loss_per_pos"], lb, rtol=LOSS_RTOL)
+        case = dict(case, meas=case["meas_masked"])
+        scale_ref = oracle_grad(make_case(c, "A", idx))
+    else:
+        scale_ref = None
     ref = oracle_grad(case)
     res = run_gpu(pty, case, want_dz=cfg.Nz > 1)
     # intensities element by element (forward output), relative to the pattern's peak
@@ -98,7 +118,7 @@ def test_parity_all_configs(pty, c, which, B):
                                             case["meas"], geom_of(cfg)) if B <= 8 else (None, None, None)
     if I_ref is not None:
         assert np.max(np.abs(res["intensity"] - I_ref)) <= 1e-4 * I_ref.max()
-    errs = check_against_oracle(res, ref, case)
+    errs = check_against_oracle(res, ref, case, scale_ref)
     print(f"c{c}{which} B={B}: loss rel {abs(res['loss'][0]-ref['loss'])/ref['loss']:.2e} " +
           " ".join(f"{k} {v:.2e}" for k, v in errs.items()))
 
@@ -272,8 +292,9 @@ def test_adam_update_kernel_single_step(pty):
         m = (0.1 * rng.standard_normal(n)).astype(np.float32)
         v = (0.01 * rng.random(n)).astype(np.float32)
         tth, tg, tm, tv = dev(th), dev(g), dev(m), dev(v)
-        plan.adam_update(tth, tg, tm, tv, lr=5e-4, t=3)
-        rth, rm, rv = oracle.adam_step(th, g, m, v, 3, lr=5e-4)
+        b1, b2, lr = float(np.float32(0.9)), float(np.float32(0.999)), float(np.float32(5e-4))
+        plan.adam_update(tth, tg, tm, tv, lr=lr, beta1=b1, beta2=b2, t=3)
+        rth, rm, rv = oracle.adam_step(th, g, m, v, 3, lr=lr, beta1=b1, beta2=b2)
         np.testing.assert_allclose(tth.cpu().numpy(), rth, rtol=2e-6, atol=1e-9)
         np.testing.assert_allclose(tm.cpu().numpy(), rm, rtol=2e-6, atol=1e-12)
         np.testing.assert_allclose(tv.cpu().numpy(), rv, rtol=2e-6, atol=1e-12)
