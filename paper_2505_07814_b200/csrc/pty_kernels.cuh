@@ -45,27 +45,25 @@ template <int N> PTY_DEV float kp_of(int j) { return (float)(j < N / 2 ? j : j -
 
 // --------------------------------------------------------------------------- per-CTA set-up (a1)
 // F1: r = floor(p + 0.5), Delta = p - r; tables: twiddles, shift factors E (F2), propagator (F4).
-template <class SH>
-PTY_DEV void setup_tables(const Cta<SH>& c, const KArgs& A, int b, int& ry, int& rx) {
-    constexpr int N = SH::N;
+template <int N, int NT>
+PTY_DEV void setup_factors(int tid, float2* Ey, float2* Ex, float2* My, float2* Mx, float* red, const KArgs& A,
+                           int b, int& ry, int& rx) {
     const double py = (double)A.positions[2 * b], px = (double)A.positions[2 * b + 1];
     const double fy = floor(py + 0.5), fx = floor(px + 0.5);
     const float dy = (float)(py - fy), dxp = (float)(px - fx);
     int iy = (int)fy, ix = (int)fx;
     const int cy = min(max(iy, 0), A.H - N), cx = min(max(ix, 0), A.W - N);
-    if ((cy != iy || cx != ix) && c.tid == 0) flag_or(A.flags, 1);
+    if ((cy != iy || cx != ix) && tid == 0) flag_or(A.flags, 1);
     ry = cy; rx = cx;
     double ty = 0.0, tx = 0.0;
     if (A.tilt_mode == 2) { ty = (double)A.tilt[2 * b]; tx = (double)A.tilt[2 * b + 1]; }
-    for (int j = c.tid; j < N; j += SH::NT) {
+    for (int j = tid; j < N; j += NT) {
         float s, co;
-        sincospi_f(2.0f * (float)j / (float)N, &s, &co);
-        c.tw[j] = make_float2(co, -s);
         const float kp = kp_of<N>(j);
         sincospi_f(-2.0f * kp * dy, &s, &co);
-        c.Ey[j] = make_float2(co, s);
+        Ey[j] = make_float2(co, s);
         sincospi_f(-2.0f * kp * dxp, &s, &co);
-        c.Ex[j] = make_float2(co * (1.0f / N), s * (1.0f / N));
+        Ex[j] = make_float2(co * (1.0f / N), s * (1.0f / N));
         float2 my, mx;
         if (A.tilt_mode == 2) {
             const double k = (double)kp / (double)A.dx;
@@ -78,10 +76,21 @@ PTY_DEV void setup_tables(const Cta<SH>& c, const KArgs& A, int b, int& ry, int&
             my = A.prop_y[j];
             mx = A.prop_x[j];
         }
-        c.My[j] = my;
-        c.Mx[j] = make_float2(mx.x * (1.0f / (N * N)), mx.y * (1.0f / (N * N)));
+        My[j] = my;
+        Mx[j] = make_float2(mx.x * (1.0f / (N * N)), mx.y * (1.0f / (N * N)));
     }
-    if (c.tid < 64) c.red[c.tid] = 0.f;
+    if (tid < 64) red[tid] = 0.f;
+}
+
+template <class SH>
+PTY_DEV void setup_tables(const Cta<SH>& c, const KArgs& A, int b, int& ry, int& rx) {
+    constexpr int N = SH::N;
+    setup_factors<N, SH::NT>(c.tid, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
+    for (int j = c.tid; j < N; j += SH::NT) {
+        float s, co;
+        sincospi_f(2.0f * (float)j / (float)N, &s, &co);
+        c.tw[j] = make_float2(co, -s);
+    }
     pty_cta_sync();
 }
 

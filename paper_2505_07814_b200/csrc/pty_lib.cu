@@ -2,6 +2,7 @@
 // sm_100a only; no cuFFT, no CPU fallback: every step of the hot path runs in the kernels here.
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -9,6 +10,7 @@
 
 #include "../../include/pty.h"
 #include "pty_kernels.cuh"
+#include "pty_kernels128.cuh"
 
 namespace cg = cooperative_groups;
 using namespace pty;
@@ -51,6 +53,27 @@ __global__ void __launch_bounds__(SH::NT, MinBlocks<SH>::value) pty_bwd_kernel(c
     Cta<SH> c = make_cta<SH>(smem);
     if constexpr (SH::CL > 1) cg::this_cluster().sync();
     bwd_body<SH>(A, c, blockIdx.x / SH::CL);
+}
+
+// N = 128 on the register-resident FFT (pty_fft128.cuh): the default path for the headline config
+__device__ __forceinline__ Cta128 make_cta128(unsigned char* smem) {
+    Cta128 c;
+    c.tid = threadIdx.x;
+    c.X = reinterpret_cast<float2*>(smem);
+    float2* tab = reinterpret_cast<float2*>(smem + F128::xch_bytes);
+    c.twy = tab; c.twx = tab + 128; c.Ey = tab + 256; c.Ex = tab + 384; c.My = tab + 512; c.Mx = tab + 640;
+    c.red = reinterpret_cast<float*>(tab + 768);
+    return c;
+}
+
+__global__ void __launch_bounds__(F128::NT, 1) pty_fwd128_kernel(const KArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    fwd_body128(A, make_cta128(smem), blockIdx.x);
+}
+
+__global__ void __launch_bounds__(F128::NT, 1) pty_bwd128_kernel(const KArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    bwd_body128(A, make_cta128(smem), blockIdx.x);
 }
 
 template <class SH, int DIR>
@@ -237,6 +260,7 @@ struct pty_plan {
     const void *f_object, *f_probe, *f_positions, *f_tilt, *f_meas;
     int32_t f_B;
 
+    bool reg128;                 // N = 128 on the register-resident FFT (default) or the shared-memory passes
     // optional kernel timing (pty_profile)
     bool profiling;
     struct Timed { cudaEvent_t a, b; int which; };
@@ -324,10 +348,14 @@ struct ScopedTimer {
 
 template <class SH> cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 0, st);
+    if (SH::N == 128 && p->reg128)
+        return launch(p, pty_fwd128_kernel, A.B * A.M, F128::NT, F128::smem_bytes, 1, st, A);
     return launch(p, pty_fwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
 template <class SH> cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 1, st);
+    if (SH::N == 128 && p->reg128)
+        return launch(p, pty_bwd128_kernel, A.B * A.M, F128::NT, F128::smem_bytes, 1, st, A);
     return launch(p, pty_bwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
 
@@ -486,6 +514,13 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
         return fail(nullptr, PTY_ERR_UNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor);
     }
     if (e == cudaSuccess) e = PTY_DISPATCH_N(p, set_smem_attrs<Shape<64>>(), set_smem_attrs<Shape<128>>(), set_smem_attrs<Shape<256>>());
+    const char* sel = getenv("PTY_FFT128");          // "smem" selects the shared-memory-pass kernels for N = 128
+    p->reg128 = !(sel && strcmp(sel, "smem") == 0);
+    if (e == cudaSuccess && dims->N == 128) {
+        e = cudaFuncSetAttribute(pty_fwd128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_bwd128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
+    }
     if (e == cudaSuccess) e = cudaMemset(p->ws + L.scalars, 0, 256);
     if (e != cudaSuccess) {
         delete p;

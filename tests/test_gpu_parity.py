@@ -296,8 +296,8 @@ def test_adam_update_kernel_single_step(pty):
         plan.adam_update(tth, tg, tm, tv, lr=lr, beta1=b1, beta2=b2, t=3)
         rth, rm, rv = oracle.adam_step(th, g, m, v, 3, lr=lr, beta1=b1, beta2=b2)
         np.testing.assert_allclose(tth.cpu().numpy(), rth, rtol=2e-6, atol=2e-8)
-        np.testing.assert_allclose(tm.cpu().numpy(), rm, rtol=2e-6, atol=1e-12)
-        np.testing.assert_allclose(tv.cpu().numpy(), rv, rtol=2e-6, atol=1e-12)
+        np.testing.assert_allclose(tm.cpu().numpy(), rm, rtol=2e-6, atol=2e-7 * np.abs(rm).max())
+        np.testing.assert_allclose(tv.cpu().numpy(), rv, rtol=2e-6, atol=2e-7 * np.abs(rv).max())
 
 
 def test_pty_step_matches_oracle_adam_over_steps(pty):
