@@ -1,4 +1,4 @@
-// pty_fft128.cuh -- register-resident 128 x 128 2-D FFT for one CTA of 512 threads.
+// pty_fft128.cuh -- register-resident 128 x 128 2-D FFT for one CTA of 512 threads, in-place exchange.
 //
 // The whole wave lives in registers (32 complex values per thread); shared memory is only the
 // exchange space between register phases.  A forward transform runs three phases (decimation in
@@ -9,20 +9,29 @@
 // TWO shared-memory exchanges per 2-D FFT, and every pointwise step of the method (object multiply,
 // propagator, seeds, gradient products) is done on registers.
 //
+// IN-PLACE EXCHANGE.  Every element has ONE home slot in the exchange array X[128][P]:
+//     slot(rho, c) = rho * P + 17 (c >> 4) + (c & 15),        P = 136 float2
+// where (rho, c) = (4 k1y + q, x) between phases 1 and 2 and (4 k1y + k2y, 16 k1x + n2x) between
+// phases 2 and 3.  In each phase a thread reads its 32 slots, transforms, and writes its results
+// back to THE SAME 32 slots, so a slot is never touched by two threads between two barriers: one
+// CTA barrier per exchange (two per 2-D FFT) is enough, no barrier separates a phase's loads from
+// its stores, and the loads of a phase can be consumed as they arrive.
+//
 // Index split:  y = 4 n1 + q      (n1 < 32, q < 4)        ky = k1y + 32 k2y   (k1y < 32, k2y < 4)
 //               x = 16 n1x + n2x  (n1x < 8, n2x < 16)     kx = k1x + 8 k2x    (k1x < 8,  k2x < 16)
 //
-//   L1: thread (q = tid >> 7, x = tid & 127)            holds a[y = 4 n1 + q][x],            n1  = 0..31
-//   L2: thread (k1y = tid >> 4, n2x = tid & 15)         holds (q | k2y) x (n1x | k1x),       4 x 8
-//   L3: thread (k1x = tid & 7, ky0 = tid >> 3)          holds A[ky0 + 64 j][k1x + 8 k2x],    j < 2, k2x < 16
+//   L1: thread (q = tid >> 7, x = tid & 127)      holds a[y = 4 n1 + q][x],             n1 = 0..31
+//   L2: thread (k1y = tid >> 4, n2x = tid & 15)   holds (q | k2y) x (n1x | k1x),        4 x 8
+//   L3: thread (k1x = tid & 7, kyl = tid >> 3)    holds rows rho = kyl + 64 j, j < 2, i.e.
+//        A[ky = (kyl >> 2) + 16 j + 32 (kyl & 3)][kx = k1x + 8 k2x],  k2x < 16,  register 16 j + k2x
 //
-//   forward:  radix-32 over n1, twiddle W128^(q k1y) | X1 | radix-4 over q, radix-8 over n1x,
-//             twiddle W128^(n2x k1x) | X2 | radix-16 over n2x.
+//   forward:  radix-32 over n1 | X | twiddle W128^(q k1y), radix-4 over q, radix-8 over n1x,
+//             twiddle W128^(n2x k1x) | X | radix-16 over n2x.
 //   inverse:  the same steps conjugated, in reverse order.  Both are unscaled.
 //
-// Exchange X1 is the array E1[4 k1y + q][x] (pitch 128); X2 is E2[ky][17 k1x + n2x] (pitch 136):
-// both sides of both exchanges touch 16 consecutive float2 per half-warp, or 8 lanes at stride 17
-// in two rows whose offset is 16 banks -> conflict-free 8-byte accesses.
+// Bank conflicts (8-byte accesses, one half-warp per wavefront): phase 1 touches 16 consecutive
+// float2 of one row; phase 2 the same; phase 3 touches 8 slots at stride 17 in each of two rows
+// whose offset P = 136 = 8 (mod 16) float2 -> all conflict-free.
 #pragma once
 #include "pty_fft.cuh"
 
@@ -30,10 +39,9 @@ namespace pty {
 
 struct F128 {
     static constexpr int N = 128, NT = 512;
-    static constexpr int P1 = 128;             // pitch of E1 (float2)
-    static constexpr int P2 = 136;             // pitch of E2 (float2): 8 * 17
-    static constexpr size_t xch_bytes = size_t(128) * P2 * sizeof(float2);
-    // tables: twy[4][32], twx[8][16], Ey, Ex, My, Mx [128 each], red[64]
+    static constexpr int P = 136;              // pitch of X (float2): 8 * 17
+    static constexpr size_t xch_bytes = size_t(128) * P * sizeof(float2);
+    // tables: twy[32][4], twx[8][16], Ey, Ex, My, Mx [128 each], red[64]
     static constexpr size_t table_bytes = (128 + 128 + 4 * 128) * sizeof(float2) + 64 * sizeof(float);
     static constexpr size_t smem_bytes = xch_bytes + table_bytes;
 };
@@ -41,7 +49,7 @@ struct F128 {
 struct Cta128 {
     int tid;
     float2* X;                       // exchange space
-    float2 *twy, *twx;               // W128^(q k1y) [4][32];  W128^(n2x k1x) [8][16]   (forward sign)
+    float2 *twy, *twx;               // W128^(q k1y) [32][4];  W128^(n2x k1x) [8][16]   (forward sign)
     float2 *Ey, *Ex, *My, *Mx;       // [128] shift and propagator factors (Ex carries 1/N, Mx 1/N^2)
     float* red;
     // L1 coordinates
@@ -49,7 +57,12 @@ struct Cta128 {
     PTY_DEV int x() const { return tid & 127; }
     // L3 coordinates
     PTY_DEV int k1x() const { return tid & 7; }
-    PTY_DEV int ky0() const { return tid >> 3; }
+    PTY_DEV int kyl() const { return tid >> 3; }
+    PTY_DEV int ky(int j) const { const int l = tid >> 3; return (l >> 2) + 16 * j + 32 * (l & 3); }
+    // home slots
+    PTY_DEV float2* slot1() const { return X + (tid >> 7) * F128::P + 17 * ((tid & 127) >> 4) + (tid & 15); }   // + 4 k P
+    PTY_DEV float2* slot2() const { return X + 4 * (tid >> 4) * F128::P + (tid & 15); }                         // + q P + 17 n1x
+    PTY_DEV float2* slot3() const { return X + (tid >> 3) * F128::P + 17 * (tid & 7); }                         // + 64 j P + n2
 };
 
 // cos / sin of 2 pi j / 32
@@ -96,7 +109,7 @@ template <int DIR> PTY_DEV void fft32(float2 (&v)[32]) {
 PTY_DEV void f128_fill_twiddles(const Cta128& c) {
     for (int i = c.tid; i < 128; i += F128::NT) {
         float s, co;
-        const int qq = i >> 5, k1y = i & 31;
+        const int k1y = i >> 2, qq = i & 3;
         sincospi_f(2.0f * (float)(qq * k1y) / 128.0f, &s, &co);
         c.twy[i] = make_float2(co, -s);
         const int k1 = i >> 4, n2 = i & 15;
@@ -105,63 +118,53 @@ PTY_DEV void f128_fill_twiddles(const Cta128& c) {
     }
 }
 
-template <int DIR> PTY_DEV float2 tw_dir(float2 w) { return DIR < 0 ? w : make_float2(w.x, -w.y); }
+// a * w (DIR < 0) or a * conj(w) (DIR > 0), w a forward-sign twiddle
+template <int DIR> PTY_DEV float2 mul_tw(float2 a, float2 w) { return DIR < 0 ? cmul(a, w) : cmulc(w, a); }
 
 // ------------------------------------------------------------------------------ forward, L1 -> L3
-// in: v[n1] = a[4 n1 + q][x];  out: v[16 j + k2x] = A[ky0 + 64 j][k1x + 8 k2x]  (unscaled).
-// The caller guarantees nobody is still reading the exchange space (a CTA barrier sits at the end
-// of every transform).
+// in: v[n1] = a[4 n1 + q][x];  out: v[16 j + k2x] = A[ky(j)][k1x + 8 k2x]  (unscaled).
+// No barrier is needed before the first store: the slots written here were last read by this thread.
 PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) {
     constexpr int DIR = -1;
-    {   // phase 1 (L1): radix-32 over n1, twiddle W128^(q k1y), write E1[4 k1y + q][x]
+    constexpr int P = F128::P;
+    {   // phase 1 (L1): radix-32 over n1, store to the home slots
         fft32<DIR>(v);
-        const int q = c.q(), x = c.x();
-        if (q != 0) {
-            const float2* tw = c.twy + 32 * q;
+        float2* s1 = c.slot1();
 #pragma unroll
-            for (int k = 1; k < 32; ++k) v[k] = cmul(v[k], tw[k]);
-        }
-#pragma unroll
-        for (int k = 0; k < 32; ++k) c.X[(4 * k + q) * F128::P1 + x] = v[k];
+        for (int k = 0; k < 32; ++k) s1[4 * k * P] = v[k];
     }
     pty_cta_sync();
-    {   // phase 2 (L2): radix-4 over q, radix-8 over n1x, twiddle W128^(n2x k1x), write E2
-        const int k1y = c.tid >> 4, n2x = c.tid & 15;
+    {   // phase 2 (L2): twiddle W128^(q k1y), radix-4 over q, radix-8 over n1x, twiddle W128^(n2x k1x)
+        float2* s2 = c.slot2();
+        const float2* ty = c.twy + 4 * (c.tid >> 4);
+        const float2 wy1 = ty[1], wy2 = ty[2], wy3 = ty[3];
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-#pragma unroll
-            for (int n1x = 0; n1x < 8; ++n1x) v[8 * q + n1x] = c.X[(4 * k1y + q) * F128::P1 + 16 * n1x + n2x];
-        pty_cta_sync();
-#pragma unroll
-        for (int n1x = 0; n1x < 8; ++n1x) bfly4<DIR>(v[n1x], v[8 + n1x], v[16 + n1x], v[24 + n1x]);   // -> v[8 k2y + n1x]
-        float2 tw[8];
-#pragma unroll
-        for (int k1 = 1; k1 < 8; ++k1) tw[k1] = c.twx[16 * k1 + n2x];
+        for (int n1x = 0; n1x < 8; ++n1x) {
+            float2 a0 = s2[17 * n1x], a1 = s2[P + 17 * n1x], a2 = s2[2 * P + 17 * n1x], a3 = s2[3 * P + 17 * n1x];
+            a1 = cmul(a1, wy1); a2 = cmul(a2, wy2); a3 = cmul(a3, wy3);
+            bfly4<DIR>(a0, a1, a2, a3);
+            v[n1x] = a0; v[8 + n1x] = a1; v[16 + n1x] = a2; v[24 + n1x] = a3;       // -> v[8 k2y + n1x]
+        }
+        const float2* tx = c.twx + (c.tid & 15);
 #pragma unroll
         for (int k2y = 0; k2y < 4; ++k2y) {
             float2 w[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) w[i] = v[8 * k2y + i];
             RegFFT<8, DIR>::run(w);
-            float2* row = c.X + (k1y + 32 * k2y) * F128::P2 + n2x;
-            row[0] = w[0];
+            s2[k2y * P] = w[0];
 #pragma unroll
-            for (int k1 = 1; k1 < 8; ++k1) row[17 * k1] = cmul(w[k1], tw[k1]);
+            for (int k1 = 1; k1 < 8; ++k1) s2[k2y * P + 17 * k1] = cmul(w[k1], tx[16 * k1]);
         }
     }
     pty_cta_sync();
     {   // phase 3 (L3): radix-16 over n2x
-        const int k1x = c.k1x(), ky0 = c.ky0();
-#pragma unroll
-        for (int j = 0; j < 2; ++j)
-#pragma unroll
-            for (int n2 = 0; n2 < 16; ++n2) v[16 * j + n2] = c.X[(ky0 + 64 * j) * F128::P2 + 17 * k1x + n2];
-        pty_cta_sync();
+        const float2* s3 = c.slot3();
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
             float2 w[16];
 #pragma unroll
-            for (int i = 0; i < 16; ++i) w[i] = v[16 * j + i];
+            for (int i = 0; i < 16; ++i) w[i] = s3[64 * j * P + i];
             RegFFT<16, DIR>::run(w);
 #pragma unroll
             for (int i = 0; i < 16; ++i) v[16 * j + i] = w[i];
@@ -170,41 +173,35 @@ PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) {
 }
 
 // ------------------------------------------------------------------------------ inverse, L3 -> L1
-// in: v[16 j + k2x] = A[ky0 + 64 j][k1x + 8 k2x];  out: v[n1] = a[4 n1 + q][x]  (unscaled: x N^2).
+// in: v[16 j + k2x] = A[ky(j)][k1x + 8 k2x];  out: v[n1] = a[4 n1 + q][x]  (unscaled: x N^2).
 // MY: 0 none, +1 multiply the spectrum by My[ky], -1 by conj(My[ky]) (the k_y factor of the
 // propagator, applied where every thread sees only 4 distinct ky).
 template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) {
     constexpr int DIR = +1;
-    {   // phase 3' (L3): inverse radix-16 over k2x, write E2[ky][17 k1x + n2x]
-        const int k1x = c.k1x(), ky0 = c.ky0();
+    constexpr int P = F128::P;
+    {   // phase 3' (L3): inverse radix-16 over k2x, store to the home slots
+        float2* s3 = c.slot3();
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
             float2 w[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) w[i] = v[16 * j + i];
             RegFFT<16, DIR>::run(w);
-            float2* row = c.X + (ky0 + 64 * j) * F128::P2 + 17 * k1x;
 #pragma unroll
-            for (int i = 0; i < 16; ++i) row[i] = w[i];
+            for (int i = 0; i < 16; ++i) s3[64 * j * P + i] = w[i];
         }
     }
     pty_cta_sync();
-    {   // phase 2' (L2): conj twiddle, inverse radix-8 over k1x, (My), inverse radix-4 over k2y, write E1
-        const int k1y = c.tid >> 4, n2x = c.tid & 15;
-#pragma unroll
-        for (int k2y = 0; k2y < 4; ++k2y)
-#pragma unroll
-            for (int k1 = 0; k1 < 8; ++k1) v[8 * k2y + k1] = c.X[(k1y + 32 * k2y) * F128::P2 + 17 * k1 + n2x];
-        pty_cta_sync();
-        float2 tw[8];
-#pragma unroll
-        for (int k1 = 1; k1 < 8; ++k1) tw[k1] = c.twx[16 * k1 + n2x];
+    {   // phase 2' (L2): conj twiddle, inverse radix-8 over k1x, (My), inverse radix-4 over k2y, conj twiddle
+        float2* s2 = c.slot2();
+        const int k1y = c.tid >> 4;
+        const float2* tx = c.twx + (c.tid & 15);
 #pragma unroll
         for (int k2y = 0; k2y < 4; ++k2y) {
             float2 w[8];
-            w[0] = v[8 * k2y];
+            w[0] = s2[k2y * P];
 #pragma unroll
-            for (int k1 = 1; k1 < 8; ++k1) w[k1] = cmulc(tw[k1], v[8 * k2y + k1]);
+            for (int k1 = 1; k1 < 8; ++k1) w[k1] = cmulc(tx[16 * k1], s2[k2y * P + 17 * k1]);
             RegFFT<8, DIR>::run(w);
             if (MY != 0) {
                 float2 m = c.My[k1y + 32 * k2y];
@@ -215,23 +212,27 @@ template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[8 * k2y + i] = w[i];
         }
+        const float2* ty = c.twy + 4 * k1y;
+        const float2 wy1 = ty[1], wy2 = ty[2], wy3 = ty[3];
 #pragma unroll
         for (int n1x = 0; n1x < 8; ++n1x) {
-            bfly4<DIR>(v[n1x], v[8 + n1x], v[16 + n1x], v[24 + n1x]);   // -> v[8 q + n1x]
-#pragma unroll
-            for (int q = 0; q < 4; ++q) c.X[(4 * k1y + q) * F128::P1 + 16 * n1x + n2x] = v[8 * q + n1x];
+            float2 a0 = v[n1x], a1 = v[8 + n1x], a2 = v[16 + n1x], a3 = v[24 + n1x];
+            bfly4<DIR>(a0, a1, a2, a3);                                              // -> q = 0..3
+            s2[17 * n1x] = a0;
+            s2[P + 17 * n1x] = cmulc(wy1, a1);
+            s2[2 * P + 17 * n1x] = cmulc(wy2, a2);
+            s2[3 * P + 17 * n1x] = cmulc(wy3, a3);
         }
     }
     pty_cta_sync();
-    {   // phase 1' (L1): conj twiddle W128^(-q k1y), inverse radix-32 over k1y
-        const int q = c.q(), x = c.x();
+    {   // phase 1' (L1): inverse radix-32 over k1y
+        const float2* s1 = c.slot1();
 #pragma unroll
-        for (int k = 0; k < 32; ++k) v[k] = c.X[(4 * k + q) * F128::P1 + x];
-        pty_cta_sync();
-        if (q != 0) {
-            const float2* tw = c.twy + 32 * q;
-#pragma unroll
-            for (int k = 1; k < 32; ++k) v[k] = cmulc(tw[k], v[k]);
+        for (int n2 = 0; n2 < 8; ++n2) {         // in the order the first butterflies consume them
+            v[n2] = s1[4 * n2 * P];
+            v[8 + n2] = s1[4 * (8 + n2) * P];
+            v[16 + n2] = s1[4 * (16 + n2) * P];
+            v[24 + n2] = s1[4 * (24 + n2) * P];
         }
         fft32<DIR>(v);
     }

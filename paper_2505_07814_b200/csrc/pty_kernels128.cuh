@@ -1,7 +1,7 @@
 // pty_kernels128.cuh -- forward and adjoint bodies for N = 128 on the register-resident FFT
 // (pty_fft128.cuh): one CTA of 512 threads per (position b, probe mode m); the wave stays in
 // registers through the whole slice chain, every pointwise step of the method runs on registers in
-// layout L1 (real space: rows y = 4 n1 + q of column x) or L3 (k space: ky0 + 64 j, k1x + 8 k2x).
+// layout L1 (real space: rows y = 4 n1 + q of column x) or L3 (k space: ky(j), k1x + 8 k2x; pty_fft128.cuh).
 //
 // Workspace layouts: psi (incident waves) natural [y][x]; Psi (far field) and the kept spectra in
 // "thread order" [register][tid] (private to these kernels, perfectly coalesced).
@@ -31,13 +31,13 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     setup128(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)b * A.M + m;
-    const int q = c.q(), x = c.x(), k1x = c.k1x(), ky0 = c.ky0();
+    const int q = c.q(), x = c.x(), k1x = c.k1x();
     float2 v[32];
     {   // a2: psi_0 = F^-1[E . P^]   (L3 -> L1)
         const float2* Ph = A.probe_hat + (size_t)m * NN;
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-            const int ky = ky0 + 64 * j;
+            const int ky = c.ky(j);
             const float2 ey = c.Ey[ky];
 #pragma unroll
             for (int k2 = 0; k2 < 16; ++k2) {
@@ -82,7 +82,7 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     for (int r = 0; r < 32; ++r) {
         const float2 p = cscale(v[r], 1.0f / N);
         st_stream2(Psi + r * F128::NT, p);
-        red_add(Ib + (ky0 + 64 * (r >> 4)) * N + k1x + 8 * (r & 15), p.x * p.x + p.y * p.y);
+        red_add(Ib + c.ky(r >> 4) * N + k1x + 8 * (r & 15), p.x * p.x + p.y * p.y);
     }
 }
 
@@ -94,7 +94,7 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
     setup128(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)b * A.M + m;
-    const int q = c.q(), x = c.x(), k1x = c.k1x(), ky0 = c.ky0();
+    const int q = c.q(), x = c.x(), k1x = c.k1x();
     float2 v[32];
     {   // a7, a8 (L3): g_Psi = 2 (1 - a / sqrt(I)) Psi, g_phi = F^-1[g_Psi]
         const float2* Psi = A.ws_Psi + bm * NN + c.tid;
@@ -105,7 +105,7 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
             float iv[8], av[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const int r = h + i, idx = (ky0 + 64 * (r >> 4)) * N + k1x + 8 * (r & 15);
+                const int r = h + i, idx = c.ky(r >> 4) * N + k1x + 8 * (r & 15);
                 v[r] = ld_stream2(Psi + r * F128::NT);
                 iv[i] = ldg1(Ib + idx);
                 av[i] = ldg1(ab + idx);
@@ -147,7 +147,7 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
                 const float2* hat = A.ws_hat + (bm * (A.Nz - 1) + (s - 1)) * NN + c.tid;
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
-                    const int ky = ky0 + 64 * j;
+                    const int ky = c.ky(j);
                     const float2 my = c.My[ky];
                     const float kyf = kp_of<N>(ky);
 #pragma unroll
@@ -173,7 +173,7 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
     float accy = 0.f, accx = 0.f;
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
-        const int ky = ky0 + 64 * j;
+        const int ky = c.ky(j);
         const float2 ey = c.Ey[ky];
         const float kyf = kp_of<N>(ky);
 #pragma unroll
