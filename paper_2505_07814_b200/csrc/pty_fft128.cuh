@@ -41,8 +41,8 @@ struct F128 {
     static constexpr int N = 128, NT = 512;
     static constexpr int P = 136;              // pitch of X (float2): 8 * 17
     static constexpr size_t xch_bytes = size_t(128) * P * sizeof(float2);
-    // tables: twy[32][4], twx[8][16], Ey, Ex, My, Mx [128 each], red[64]
-    static constexpr size_t table_bytes = (128 + 128 + 4 * 128) * sizeof(float2) + 64 * sizeof(float);
+    // tables: twy[32][4], twx[8][16], Ey, Ex, My, Mx [128 each], red[64], tensor-memory base
+    static constexpr size_t table_bytes = (128 + 128 + 4 * 128) * sizeof(float2) + 64 * sizeof(float) + 16;
     static constexpr size_t smem_bytes = xch_bytes + table_bytes;
 };
 
@@ -52,6 +52,7 @@ struct Cta128 {
     float2 *twy, *twx;               // W128^(q k1y) [32][4];  W128^(n2x k1x) [8][16]   (forward sign)
     float2 *Ey, *Ex, *My, *Mx;       // [128] shift and propagator factors (Ex carries 1/N, Mx 1/N^2)
     float* red;
+    unsigned tm;                     // tensor-memory address of this thread's 128-column staging block
     // L1 coordinates
     PTY_DEV int q() const { return tid >> 7; }
     PTY_DEV int x() const { return tid & 127; }
@@ -118,17 +119,24 @@ PTY_DEV void f128_fill_twiddles(const Cta128& c) {
     }
 }
 
+// Background work interleaved with a transform: the transforms call bg.tick<K>() at 8 points spread
+// evenly over their arithmetic (K = 0..7 in program order); the kernel bodies use the ticks to fetch
+// the global data of the NEXT pointwise step in small chunks and park it in tensor memory.
+struct NoBg { template <int K> PTY_DEV void tick() {} };
+
 // a * w (DIR < 0) or a * conj(w) (DIR > 0), w a forward-sign twiddle
 template <int DIR> PTY_DEV float2 mul_tw(float2 a, float2 w) { return DIR < 0 ? cmul(a, w) : cmulc(w, a); }
 
 // ------------------------------------------------------------------------------ forward, L1 -> L3
 // in: v[n1] = a[4 n1 + q][x];  out: v[16 j + k2x] = A[ky(j)][k1x + 8 k2x]  (unscaled).
 // No barrier is needed before the first store: the slots written here were last read by this thread.
-PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) {
+template <class BG> PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32], BG& bg) {
     constexpr int DIR = -1;
     constexpr int P = F128::P;
     {   // phase 1 (L1): radix-32 over n1, store to the home slots
+        bg.template tick<0>();
         fft32<DIR>(v);
+        bg.template tick<1>();
         float2* s1 = c.slot1();
 #pragma unroll
         for (int k = 0; k < 32; ++k) s1[4 * k * P] = v[k];
@@ -144,7 +152,9 @@ PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) {
             a1 = cmul(a1, wy1); a2 = cmul(a2, wy2); a3 = cmul(a3, wy3);
             bfly4<DIR>(a0, a1, a2, a3);
             v[n1x] = a0; v[8 + n1x] = a1; v[16 + n1x] = a2; v[24 + n1x] = a3;       // -> v[8 k2y + n1x]
+            if (n1x == 3) bg.template tick<2>();
         }
+        bg.template tick<3>();
         const float2* tx = c.twx + (c.tid & 15);
 #pragma unroll
         for (int k2y = 0; k2y < 4; ++k2y) {
@@ -155,7 +165,9 @@ PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) {
             s2[k2y * P] = w[0];
 #pragma unroll
             for (int k1 = 1; k1 < 8; ++k1) s2[k2y * P + 17 * k1] = cmul(w[k1], tx[16 * k1]);
+            if (k2y == 1) bg.template tick<4>();
         }
+        bg.template tick<5>();
     }
     pty_cta_sync();
     {   // phase 3 (L3): radix-16 over n2x
@@ -168,15 +180,17 @@ PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) {
             RegFFT<16, DIR>::run(w);
 #pragma unroll
             for (int i = 0; i < 16; ++i) v[16 * j + i] = w[i];
+            if (j == 0) bg.template tick<6>(); else bg.template tick<7>();
         }
     }
 }
+PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_forward(c, v, bg); }
 
 // ------------------------------------------------------------------------------ inverse, L3 -> L1
 // in: v[16 j + k2x] = A[ky(j)][k1x + 8 k2x];  out: v[n1] = a[4 n1 + q][x]  (unscaled: x N^2).
 // MY: 0 none, +1 multiply the spectrum by My[ky], -1 by conj(My[ky]) (the k_y factor of the
 // propagator, applied where every thread sees only 4 distinct ky).
-template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) {
+template <int MY, class BG> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32], BG& bg) {
     constexpr int DIR = +1;
     constexpr int P = F128::P;
     {   // phase 3' (L3): inverse radix-16 over k2x, store to the home slots
@@ -189,6 +203,7 @@ template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) {
             RegFFT<16, DIR>::run(w);
 #pragma unroll
             for (int i = 0; i < 16; ++i) s3[64 * j * P + i] = w[i];
+            if (j == 0) bg.template tick<0>(); else bg.template tick<1>();
         }
     }
     pty_cta_sync();
@@ -211,7 +226,9 @@ template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) {
             }
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[8 * k2y + i] = w[i];
+            if (k2y == 1) bg.template tick<2>();
         }
+        bg.template tick<3>();
         const float2* ty = c.twy + 4 * k1y;
         const float2 wy1 = ty[1], wy2 = ty[2], wy3 = ty[3];
 #pragma unroll
@@ -222,7 +239,9 @@ template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) {
             s2[P + 17 * n1x] = cmulc(wy1, a1);
             s2[2 * P + 17 * n1x] = cmulc(wy2, a2);
             s2[3 * P + 17 * n1x] = cmulc(wy3, a3);
+            if (n1x == 3) bg.template tick<4>();
         }
+        bg.template tick<5>();
     }
     pty_cta_sync();
     {   // phase 1' (L1): inverse radix-32 over k1y
@@ -234,8 +253,11 @@ template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) {
             v[16 + n2] = s1[4 * (16 + n2) * P];
             v[24 + n2] = s1[4 * (24 + n2) * P];
         }
+        bg.template tick<6>();
         fft32<DIR>(v);
+        bg.template tick<7>();
     }
 }
+template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_inverse<MY>(c, v, bg); }
 
 }  // namespace pty

@@ -23,6 +23,31 @@ PTY_DEV void block_accumulate128(const Cta128& c, int slot, float v) {
     if (warp_leader()) red_add_shared(c.red + slot, v);
 }
 
+// ------------------------------------------------------------------------------ background fetches
+// Fetch 32 float2 per thread (rows n1 = 0..31 at stride `stride` float2 from p) into tensor memory
+// columns [tm, tm + 64), four rows per tick: tick K parks the rows fetched by tick K - 1 and issues the
+// loads of rows 4 K .. 4 K + 3.  The rows of the last tick stay in `buf` (use take<7>()).
+template <bool STREAM> struct Fetch32 {
+    const float2* p;
+    size_t stride;
+    unsigned tm;
+    float2 buf[4];
+    template <int K> PTY_DEV void tick() {
+        if (K > 0) tmem_st4(tm + 8 * (K - 1), buf);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            buf[i] = STREAM ? ld_stream2_pinned(p + (size_t)(4 * K + i) * stride) : ldg2_pinned(p + (size_t)(4 * K + i) * stride);
+    }
+    // rows 4 K .. 4 K + 3 (after the transform that ran the ticks; tmem_wait_st() once before the first)
+    template <int K> PTY_DEV void take(float2 (&o)[4]) {
+        if (K < 7) { tmem_ld4(tm + 8 * K, o); tmem_wait_ld(); }
+        else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) o[i] = buf[i];
+        }
+    }
+};
+
 // ------------------------------------------------------------------------------ forward (a2-a5)
 PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     constexpr int N = 128;
@@ -33,6 +58,11 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     const size_t bm = (size_t)b * A.M + m;
     const int q = c.q(), x = c.x(), k1x = c.k1x();
     float2 v[32];
+    // a3: the object rows of slice s are fetched during the inverse transform that precedes their use
+    Fetch32<false> fo;
+    fo.p = A.object + ((size_t)ry + q) * A.W + rx + x;
+    fo.stride = (size_t)4 * A.W;
+    fo.tm = c.tm;
     {   // a2: psi_0 = F^-1[E . P^]   (L3 -> L1)
         const float2* Ph = A.probe_hat + (size_t)m * NN;
 #pragma unroll
@@ -45,23 +75,25 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
                 v[16 * j + k2] = cmul(cmul(ldg2(Ph + ky * N + kx), ey), c.Ex[kx]);
             }
         }
-        f128_inverse<0>(c, v);
+        f128_inverse<0>(c, v, fo);
     }
     for (int s = 0; s < A.Nz; ++s) {
         {   // a3 + a4 (L1): keep psi_{s-1}, phi_s = O_b[s] psi_{s-1}
-            const float2* obj = A.object + ((size_t)s * A.H + ry + q) * A.W + rx + x;
             float2* save = A.ws_psi + (bm * A.Nz + s) * NN + q * N + x;
-#pragma unroll
-            for (int h = 0; h < 32; h += 8) {
-                float2 o[8];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) o[i] = ldg2(obj + (size_t)(4 * (h + i)) * A.W);
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    st_stream2(save + 4 * (h + i) * N, v[h + i]);
-                    v[h + i] = cmul(v[h + i], o[i]);
-                }
+            tmem_wait_st();
+#define PTY_OBJ_CHUNK(K)                                                   \
+            {                                                              \
+                float2 o[4];                                               \
+                fo.template take<K>(o);                                    \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i) {            \
+                    st_stream2(save + 4 * (4 * K + i) * N, v[4 * K + i]);  \
+                    v[4 * K + i] = cmul(v[4 * K + i], o[i]);               \
+                }                                                          \
             }
+            PTY_OBJ_CHUNK(7) PTY_OBJ_CHUNK(0) PTY_OBJ_CHUNK(1) PTY_OBJ_CHUNK(2)
+            PTY_OBJ_CHUNK(3) PTY_OBJ_CHUNK(4) PTY_OBJ_CHUNK(5) PTY_OBJ_CHUNK(6)
+#undef PTY_OBJ_CHUNK
+            fo.p += (size_t)A.H * A.W;
         }
         f128_forward(c, v);
         if (s == A.Nz - 1) break;
@@ -73,7 +105,7 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
                 if (hat) st_stream2(hat + r * F128::NT, v[r]);
             }
         }
-        f128_inverse<+1>(c, v);
+        f128_inverse<+1>(c, v, fo);
     }
     // a5 (L3): Psi = F[phi_Nz] / N, I += |Psi|^2
     float2* Psi = A.ws_Psi + bm * NN + c.tid;

@@ -63,17 +63,35 @@ __device__ __forceinline__ Cta128 make_cta128(unsigned char* smem) {
     float2* tab = reinterpret_cast<float2*>(smem + F128::xch_bytes);
     c.twy = tab; c.twx = tab + 128; c.Ey = tab + 256; c.Ex = tab + 384; c.My = tab + 512; c.Mx = tab + 640;
     c.red = reinterpret_cast<float*>(tab + 768);
+    // tensor memory: all 512 columns, allocated by warp 0; thread block = lane quarter (warp % 4),
+    // columns [128 (warp / 4), + 128)
+    unsigned* tbase = reinterpret_cast<unsigned*>(c.red + 64);
+    if ((threadIdx.x >> 5) == 0) tmem_alloc512(tbase);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    const unsigned w = threadIdx.x >> 5;
+    c.tm = *tbase + ((32u * (w & 3u)) << 16) + 128u * (w >> 2);
     return c;
+}
+
+__device__ __forceinline__ void release_cta128(unsigned char* smem) {
+    tmem_fence_before_sync();
+    __syncthreads();
+    float2* tab = reinterpret_cast<float2*>(smem + F128::xch_bytes);
+    if ((threadIdx.x >> 5) == 0) tmem_dealloc512(*reinterpret_cast<unsigned*>(reinterpret_cast<float*>(tab + 768) + 64));
 }
 
 __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128_kernel(const KArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     fwd_body128(A, make_cta128(smem), blockIdx.x);
+    release_cta128(smem);
 }
 
 __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128_kernel(const KArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     bwd_body128(A, make_cta128(smem), blockIdx.x);
+    release_cta128(smem);
 }
 
 template <class SH, int DIR>

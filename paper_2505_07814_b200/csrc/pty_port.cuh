@@ -32,6 +32,44 @@ PTY_DEV float warp_sum(float v) {
     return v;
 }
 PTY_DEV bool warp_leader() { return (threadIdx.x & 31) == 0; }
+// ---- tensor memory (TMEM) as a per-thread staging buffer (tcgen05.st / tcgen05.ld, 32x32b shape):
+// a warp owns the 32 TMEM lanes of its sub-partition (warp id % 4); lane i of the warp reads and writes
+// TMEM lane 32 (warp % 4) + i, N consecutive 32-bit columns per instruction.  Used to park data that was
+// fetched from global memory early (no registers, no shared memory, not the LSU pipe).
+PTY_DEV void tmem_alloc512(unsigned* smem_slot) {     // one full warp
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;"
+                 ::"r"((unsigned)__cvta_generic_to_shared(smem_slot)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+PTY_DEV void tmem_dealloc512(unsigned base) {         // the same warp
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base) : "memory");
+}
+PTY_DEV void tmem_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+PTY_DEV void tmem_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+PTY_DEV void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+PTY_DEV void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+PTY_DEV void tmem_st4(unsigned ta, const float2 (&v)[4]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 ::"r"(ta), "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "f"(v[2].x), "f"(v[2].y),
+                   "f"(v[3].x), "f"(v[3].y) : "memory");
+}
+PTY_DEV void tmem_ld4(unsigned ta, float2 (&v)[4]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y),
+                   "=f"(v[3].x), "=f"(v[3].y) : "r"(ta) : "memory");
+}
+// global load that the compiler must leave where it is written (prefetch ticks)
+PTY_DEV float2 ldg2_pinned(const float2* p) {
+    float2 v;
+    asm volatile("ld.global.nc.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+PTY_DEV float2 ld_stream2_pinned(const float2* p) {
+    float2 v;
+    asm volatile("ld.global.cs.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 PTY_DEV void sincospi_f(float x, float* s, float* c) { sincospif(x, s, c); }
 PTY_DEV float rsqrt_f(float x) { return rsqrtf(x); }
 }  // namespace pty
