@@ -1,37 +1,32 @@
-// pty_fft128.cuh -- register-resident 128 x 128 2-D FFT for one CTA of 512 threads, in-place exchange.
+// pty_fft128.cuh -- register-resident 128 x 128 2-D FFT for one CTA of 512 threads on sm_100a:
+// ONE shared-memory exchange per 2-D FFT; the other two exchanges go through tensor memory (TMEM).
 //
-// The whole wave lives in registers (32 complex values per thread); shared memory is only the
-// exchange space between register phases.  A forward transform runs three phases (decimation in
-// time), its inverse runs the exact mirror (decimation in frequency), so that
-//   * the forward ENDS and the inverse STARTS in the same register layout ("L3", k space), and
-//   * the inverse ENDS and the forward STARTS in the same layout ("L1", real space).
-// A chain  ... F^-1 -> (pointwise in L1) -> F -> (pointwise in L3) -> F^-1 ...  therefore needs only
-// TWO shared-memory exchanges per 2-D FFT, and every pointwise step of the method (object multiply,
-// propagator, seeds, gradient products) is done on registers.
+// The wave lives in registers, 32 complex values per thread.  Thread id = 128 g + c (g < 4, c < 128).
+// A 1-D FFT of length 128 along one axis is split 128 = 32 x 4 (decimation in time):
+//   (a) radix-32 in registers over the 32 strided samples a thread holds,
+//   (b) an exchange among the FOUR threads that share c (they differ in g only),
+//   (c) twiddle W128^(q k1) and radix-4 over q in registers.
+// The four threads of (b) are the same lane of the four warps of one SM sub-partition, i.e. they
+// share one TMEM lane: each writes its 32 values to its own 64 TMEM columns (tcgen05.st) and reads
+// 8 values from each of the four column blocks (tcgen05.ld).  That exchange costs no shared-memory
+// bandwidth and does not go through the LSU pipe; its barrier covers the 4 warps of one sub-partition.
+// Between the two axes the wave is transposed through shared memory, in place: element (ky, x) has
+// the single home slot X[ky * 129 + x]; the y-side thread (g, x) touches it with lanes along x, the
+// x-side thread (g, ky) with lanes along ky (stride 129 float2: conflict-free), and a slot is never
+// touched by two threads between two CTA barriers.  A forward transform and its inverse are exact
+// mirrors, so a chain  F^-1 -> (pointwise, layout R) -> F -> (pointwise, layout K) -> F^-1 ...  needs one
+// CTA barrier and two or three sub-partition barriers per 2-D FFT.
 //
-// IN-PLACE EXCHANGE.  Every element has ONE home slot in the exchange array X[128][P]:
-//     slot(rho, c) = rho * P + 17 (c >> 4) + (c & 15),        P = 136 float2
-// where (rho, c) = (4 k1y + q, x) between phases 1 and 2 and (4 k1y + k2y, 16 k1x + n2x) between
-// phases 2 and 3.  In each phase a thread reads its 32 slots, transforms, and writes its results
-// back to THE SAME 32 slots, so a slot is never touched by two threads between two barriers: one
-// CTA barrier per exchange (two per 2-D FFT) is enough, no barrier separates a phase's loads from
-// its stores, and the loads of a phase can be consumed as they arrive.
+//   layout R (real space): thread (q = g, x = c)   holds a[y = 4 n1 + q][x]           in v[n1],  n1 < 32
+//   layout K (k space):    thread (g, ky = c)      holds A[ky][kx = 8 g + i + 32 k2]  in v[8 k2 + i]
 //
-// Index split:  y = 4 n1 + q      (n1 < 32, q < 4)        ky = k1y + 32 k2y   (k1y < 32, k2y < 4)
-//               x = 16 n1x + n2x  (n1x < 8, n2x < 16)     kx = k1x + 8 k2x    (k1x < 8,  k2x < 16)
-//
-//   L1: thread (q = tid >> 7, x = tid & 127)      holds a[y = 4 n1 + q][x],             n1 = 0..31
-//   L2: thread (k1y = tid >> 4, n2x = tid & 15)   holds (q | k2y) x (n1x | k1x),        4 x 8
-//   L3: thread (k1x = tid & 7, kyl = tid >> 3)    holds rows rho = kyl + 64 j, j < 2, i.e.
-//        A[ky = (kyl >> 2) + 16 j + 32 (kyl & 3)][kx = k1x + 8 k2x],  k2x < 16,  register 16 j + k2x
-//
-//   forward:  radix-32 over n1 | X | twiddle W128^(q k1y), radix-4 over q, radix-8 over n1x,
-//             twiddle W128^(n2x k1x) | X | radix-16 over n2x.
+//   forward:  fft32 over n1 | T | tw, radix-4 over q -> ky = 8 g + i + 32 k2y | S (transpose) |
+//             x = 4 n1x + xq: fft32 over n1x | T | tw, radix-4 over xq -> kx = 8 g + i + 32 k2x.
 //   inverse:  the same steps conjugated, in reverse order.  Both are unscaled.
 //
-// Bank conflicts (8-byte accesses, one half-warp per wavefront): phase 1 touches 16 consecutive
-// float2 of one row; phase 2 the same; phase 3 touches 8 slots at stride 17 in each of two rows
-// whose offset P = 136 = 8 (mod 16) float2 -> all conflict-free.
+// TMEM use: 512 columns x 128 lanes, allocated once per CTA.  Thread (g, c) owns lane c, columns
+// [128 g, 128 g + 128): the first 64 are the exchange block, the last 64 a staging buffer where the
+// kernel bodies park global data fetched early (Fetch32 in pty_kernels128.cuh).
 #pragma once
 #include "pty_fft.cuh"
 
@@ -39,31 +34,26 @@ namespace pty {
 
 struct F128 {
     static constexpr int N = 128, NT = 512;
-    static constexpr int P = 136;              // pitch of X (float2): 8 * 17
+    static constexpr int P = 129;              // pitch of X (float2)
     static constexpr size_t xch_bytes = size_t(128) * P * sizeof(float2);
-    // tables: twy[32][4], twx[8][16], Ey, Ex, My, Mx [128 each], red[64], tensor-memory base
-    static constexpr size_t table_bytes = (128 + 128 + 4 * 128) * sizeof(float2) + 64 * sizeof(float) + 16;
+    // tables: twg[4][8][4], Ey, Ex, My, Mx [128 each] (float2), red[64] (float), TMEM base (16 B)
+    static constexpr size_t table_bytes = (128 + 4 * 128) * sizeof(float2) + 64 * sizeof(float) + 16;
     static constexpr size_t smem_bytes = xch_bytes + table_bytes;
 };
 
 struct Cta128 {
     int tid;
-    float2* X;                       // exchange space
-    float2 *twy, *twx;               // W128^(q k1y) [32][4];  W128^(n2x k1x) [8][16]   (forward sign)
+    float2* X;                       // transpose space
+    float2* twg;                     // W128^(q (8 g + i)) [g][i][q]   (forward sign)
     float2 *Ey, *Ex, *My, *Mx;       // [128] shift and propagator factors (Ex carries 1/N, Mx 1/N^2)
     float* red;
-    unsigned tm;                     // tensor-memory address of this thread's 128-column staging block
-    // L1 coordinates
-    PTY_DEV int q() const { return tid >> 7; }
-    PTY_DEV int x() const { return tid & 127; }
-    // L3 coordinates
-    PTY_DEV int k1x() const { return tid & 7; }
-    PTY_DEV int kyl() const { return tid >> 3; }
-    PTY_DEV int ky(int j) const { const int l = tid >> 3; return (l >> 2) + 16 * j + 32 * (l & 3); }
-    // home slots
-    PTY_DEV float2* slot1() const { return X + (tid >> 7) * F128::P + 17 * ((tid & 127) >> 4) + (tid & 15); }   // + 4 k P
-    PTY_DEV float2* slot2() const { return X + 4 * (tid >> 4) * F128::P + (tid & 15); }                         // + q P + 17 n1x
-    PTY_DEV float2* slot3() const { return X + (tid >> 3) * F128::P + 17 * (tid & 7); }                         // + 64 j P + n2
+    unsigned tmq;                    // TMEM address of this thread's lane quarter, column 0
+    PTY_DEV int g() const { return tid >> 7; }
+    PTY_DEV int cc() const { return tid & 127; }
+    PTY_DEV unsigned tm_x() const { return tmq + 128u * (unsigned)(tid >> 7); }          // exchange block
+    PTY_DEV unsigned tm_s() const { return tmq + 128u * (unsigned)(tid >> 7) + 64u; }    // staging block
+    // layout K: k_x of register r = 8 k2 + i
+    PTY_DEV int kx(int r) const { return 8 * (tid >> 7) + (r & 7) + 32 * (r >> 3); }
 };
 
 // cos / sin of 2 pi j / 32
@@ -83,8 +73,14 @@ template <int J, int DIR> PTY_DEV float2 mul_w32(float2 a) {
     else return mul_cs<DIR>(a, c, s);
 }
 
+// Background work interleaved with a transform: the transforms call bg.tick<K>() at 8 points spread
+// over their arithmetic (K = 0..7 in program order); the kernel bodies use the ticks to fetch the
+// global data of the NEXT pointwise step in small chunks and park it in tensor memory.
+struct NoBg { template <int K> PTY_DEV void tick() {} };
+
 // 32-point DFT in registers, natural order in and out.  n = 8 n1 + n2, k = k1 + 4 k2.
-template <int DIR> PTY_DEV void fft32(float2 (&v)[32]) {
+// One tick (TK) between its two stages.
+template <int DIR, int TK, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg) {
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) bfly4<DIR>(v[n2], v[8 + n2], v[16 + n2], v[24 + n2]);   // -> v[8 k1 + n2]
 #define PTY_TW(K1, N2) v[8 * K1 + N2] = mul_w32<K1 * N2, DIR>(v[8 * K1 + N2]);
@@ -92,6 +88,7 @@ template <int DIR> PTY_DEV void fft32(float2 (&v)[32]) {
     PTY_TW(2, 1) PTY_TW(2, 2) PTY_TW(2, 3) PTY_TW(2, 4) PTY_TW(2, 5) PTY_TW(2, 6) PTY_TW(2, 7)
     PTY_TW(3, 1) PTY_TW(3, 2) PTY_TW(3, 3) PTY_TW(3, 4) PTY_TW(3, 5) PTY_TW(3, 6) PTY_TW(3, 7)
 #undef PTY_TW
+    bg.template tick<TK>();
     float2 o[32];
 #pragma unroll
     for (int k1 = 0; k1 < 4; ++k1) {
@@ -106,158 +103,143 @@ template <int DIR> PTY_DEV void fft32(float2 (&v)[32]) {
     for (int k = 0; k < 32; ++k) v[k] = o[k];
 }
 
-// twiddle tables (forward sign), filled once per CTA
+// twiddle table (forward sign), filled once per CTA: twg[g][i][q] = W128^(q (8 g + i))
 PTY_DEV void f128_fill_twiddles(const Cta128& c) {
-    for (int i = c.tid; i < 128; i += F128::NT) {
+    for (int j = c.tid; j < 128; j += F128::NT) {
         float s, co;
-        const int k1y = i >> 2, qq = i & 3;
-        sincospi_f(2.0f * (float)(qq * k1y) / 128.0f, &s, &co);
-        c.twy[i] = make_float2(co, -s);
-        const int k1 = i >> 4, n2 = i & 15;
-        sincospi_f(2.0f * (float)(k1 * n2) / 128.0f, &s, &co);
-        c.twx[i] = make_float2(co, -s);
+        const int gi = j >> 2, qq = j & 3;        // gi = 8 g + i
+        sincospi_f(2.0f * (float)(qq * gi) / 128.0f, &s, &co);
+        c.twg[j] = make_float2(co, -s);
     }
 }
 
-// Background work interleaved with a transform: the transforms call bg.tick<K>() at 8 points spread
-// evenly over their arithmetic (K = 0..7 in program order); the kernel bodies use the ticks to fetch
-// the global data of the NEXT pointwise step in small chunks and park it in tensor memory.
-struct NoBg { template <int K> PTY_DEV void tick() {} };
+// ------------------------------------------------------------------------------ TMEM exchange (T)
+// out[8 g2 + i] = (value in[8 g + i] of the thread (g2, c)),  g = this thread's group.
+// WAR: the partners' reads of the previous exchange must be complete before this thread overwrites
+// its block; pass true unless a CTA barrier has been crossed since the previous exchange.
+PTY_DEV void subpartition_sync(int tid) {      // the 4 warps {w, w+4, w+8, w+12} of one SM sub-partition
+    asm volatile("bar.sync %0, 128;" ::"r"(1 + ((tid >> 5) & 3)) : "memory");
+}
+template <bool WAR> PTY_DEV void f128_tmem_exchange(const Cta128& c, float2 (&v)[32]) {
+    if (WAR) {
+        tmem_fence_before_sync();
+        subpartition_sync(c.tid);
+        tmem_fence_after_sync();
+    }
+    const unsigned mine = c.tm_x();
+#pragma unroll
+    for (int h = 0; h < 4; ++h) tmem_st8(mine + 16 * h, v, 8 * h);
+    tmem_wait_st();
+    tmem_fence_before_sync();
+    subpartition_sync(c.tid);
+    tmem_fence_after_sync();
+    const unsigned col = 16u * (unsigned)c.g();
+#pragma unroll
+    for (int g2 = 0; g2 < 4; ++g2) tmem_ld8(c.tmq + 128u * g2 + col, v, 8 * g2);
+    tmem_wait_ld();
+}
 
-// a * w (DIR < 0) or a * conj(w) (DIR > 0), w a forward-sign twiddle
-template <int DIR> PTY_DEV float2 mul_tw(float2 a, float2 w) { return DIR < 0 ? cmul(a, w) : cmulc(w, a); }
+// ------------------------------------------------------------------------------ radix-4 stage (c)
+// forward: v[8 q + i] -> twiddle W128^(q (8 g + i)) -> radix-4 over q -> v[8 k2 + i]
+template <int T0, int T1, class BG> PTY_DEV void f128_radix4_fwd(const Cta128& c, float2 (&v)[32], BG& bg) {
+    const float4* tw = reinterpret_cast<const float4*>(c.twg + 32 * c.g());
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float4 t01 = tw[2 * i], t23 = tw[2 * i + 1];
+        float2 a0 = v[i];
+        float2 a1 = cmul(v[8 + i], make_float2(t01.z, t01.w));
+        float2 a2 = cmul(v[16 + i], make_float2(t23.x, t23.y));
+        float2 a3 = cmul(v[24 + i], make_float2(t23.z, t23.w));
+        bfly4<-1>(a0, a1, a2, a3);
+        v[i] = a0; v[8 + i] = a1; v[16 + i] = a2; v[24 + i] = a3;
+        if (i == 3) bg.template tick<T0>();
+    }
+    bg.template tick<T1>();
+}
+// inverse: v[8 k2 + i] -> inverse radix-4 over k2 -> conj twiddle -> v[8 q + i]
+template <int T0, int T1, class BG> PTY_DEV void f128_radix4_inv(const Cta128& c, float2 (&v)[32], BG& bg) {
+    const float4* tw = reinterpret_cast<const float4*>(c.twg + 32 * c.g());
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float4 t01 = tw[2 * i], t23 = tw[2 * i + 1];
+        float2 a0 = v[i], a1 = v[8 + i], a2 = v[16 + i], a3 = v[24 + i];
+        bfly4<+1>(a0, a1, a2, a3);
+        v[i] = a0;
+        v[8 + i] = cmulc(make_float2(t01.z, t01.w), a1);
+        v[16 + i] = cmulc(make_float2(t23.x, t23.y), a2);
+        v[24 + i] = cmulc(make_float2(t23.z, t23.w), a3);
+        if (i == 3) bg.template tick<T0>();
+    }
+    bg.template tick<T1>();
+}
 
-// ------------------------------------------------------------------------------ forward, L1 -> L3
-// in: v[n1] = a[4 n1 + q][x];  out: v[16 j + k2x] = A[ky(j)][k1x + 8 k2x]  (unscaled).
-// No barrier is needed before the first store: the slots written here were last read by this thread.
+// ------------------------------------------------------------------------------ forward, R -> K
+// in: v[n1] = a[4 n1 + q][x];  out: v[8 k2 + i] = A[ky = c][kx = 8 g + i + 32 k2]  (unscaled).
 template <class BG> PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32], BG& bg) {
-    constexpr int DIR = -1;
     constexpr int P = F128::P;
-    {   // phase 1 (L1): radix-32 over n1, store to the home slots
-        bg.template tick<0>();
-        fft32<DIR>(v);
-        bg.template tick<1>();
-        float2* s1 = c.slot1();
+    const int g = c.g(), cc = c.cc();
+    // y axis
+    bg.template tick<0>();
+    fft32<-1, 1>(v, bg);
+    f128_tmem_exchange<true>(c, v);
+    f128_radix4_fwd<2, 3>(c, v, bg);
+    {   // S: thread (g, x = cc) holds ky = 8 g + i + 32 k2 in v[8 k2 + i]
+        float2* s = c.X + (8 * g) * P + cc;
 #pragma unroll
-        for (int k = 0; k < 32; ++k) s1[4 * k * P] = v[k];
+        for (int r = 0; r < 32; ++r) s[((r & 7) + 32 * (r >> 3)) * P] = v[r];
     }
     pty_cta_sync();
-    {   // phase 2 (L2): twiddle W128^(q k1y), radix-4 over q, radix-8 over n1x, twiddle W128^(n2x k1x)
-        float2* s2 = c.slot2();
-        const float2* ty = c.twy + 4 * (c.tid >> 4);
-        const float2 wy1 = ty[1], wy2 = ty[2], wy3 = ty[3];
+    {   // thread (xq = g, ky = cc) takes x = 4 n1x + xq
+        const float2* s = c.X + cc * P + g;
 #pragma unroll
-        for (int n1x = 0; n1x < 8; ++n1x) {
-            float2 a0 = s2[17 * n1x], a1 = s2[P + 17 * n1x], a2 = s2[2 * P + 17 * n1x], a3 = s2[3 * P + 17 * n1x];
-            a1 = cmul(a1, wy1); a2 = cmul(a2, wy2); a3 = cmul(a3, wy3);
-            bfly4<DIR>(a0, a1, a2, a3);
-            v[n1x] = a0; v[8 + n1x] = a1; v[16 + n1x] = a2; v[24 + n1x] = a3;       // -> v[8 k2y + n1x]
-            if (n1x == 3) bg.template tick<2>();
-        }
-        bg.template tick<3>();
-        const float2* tx = c.twx + (c.tid & 15);
-#pragma unroll
-        for (int k2y = 0; k2y < 4; ++k2y) {
-            float2 w[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) w[i] = v[8 * k2y + i];
-            RegFFT<8, DIR>::run(w);
-            s2[k2y * P] = w[0];
-#pragma unroll
-            for (int k1 = 1; k1 < 8; ++k1) s2[k2y * P + 17 * k1] = cmul(w[k1], tx[16 * k1]);
-            if (k2y == 1) bg.template tick<4>();
-        }
-        bg.template tick<5>();
-    }
-    pty_cta_sync();
-    {   // phase 3 (L3): radix-16 over n2x
-        const float2* s3 = c.slot3();
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            float2 w[16];
-#pragma unroll
-            for (int i = 0; i < 16; ++i) w[i] = s3[64 * j * P + i];
-            RegFFT<16, DIR>::run(w);
-#pragma unroll
-            for (int i = 0; i < 16; ++i) v[16 * j + i] = w[i];
-            if (j == 0) bg.template tick<6>(); else bg.template tick<7>();
+        for (int n2 = 0; n2 < 8; ++n2) {     // in the order the first butterflies consume them
+            v[n2] = s[4 * n2];
+            v[8 + n2] = s[4 * (8 + n2)];
+            v[16 + n2] = s[4 * (16 + n2)];
+            v[24 + n2] = s[4 * (24 + n2)];
         }
     }
+    // x axis
+    bg.template tick<4>();
+    fft32<-1, 5>(v, bg);
+    f128_tmem_exchange<false>(c, v);
+    f128_radix4_fwd<6, 7>(c, v, bg);
 }
-PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_forward(c, v, bg); }
 
-// ------------------------------------------------------------------------------ inverse, L3 -> L1
-// in: v[16 j + k2x] = A[ky(j)][k1x + 8 k2x];  out: v[n1] = a[4 n1 + q][x]  (unscaled: x N^2).
-// MY: 0 none, +1 multiply the spectrum by My[ky], -1 by conj(My[ky]) (the k_y factor of the
-// propagator, applied where every thread sees only 4 distinct ky).
-template <int MY, class BG> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32], BG& bg) {
-    constexpr int DIR = +1;
+// ------------------------------------------------------------------------------ inverse, K -> R
+// in: v[8 k2 + i] = A[ky = c][kx = 8 g + i + 32 k2];  out: v[n1] = a[4 n1 + q][x]  (unscaled: x N^2).
+template <class BG> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32], BG& bg) {
     constexpr int P = F128::P;
-    {   // phase 3' (L3): inverse radix-16 over k2x, store to the home slots
-        float2* s3 = c.slot3();
+    const int g = c.g(), cc = c.cc();
+    // x axis
+    f128_radix4_inv<0, 1>(c, v, bg);
+    f128_tmem_exchange<true>(c, v);
+    fft32<+1, 2>(v, bg);
+    bg.template tick<3>();
+    {   // S: thread (xq = g, ky = cc) holds x = 4 n1x + xq in v[n1x]
+        float2* s = c.X + cc * P + g;
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            float2 w[16];
-#pragma unroll
-            for (int i = 0; i < 16; ++i) w[i] = v[16 * j + i];
-            RegFFT<16, DIR>::run(w);
-#pragma unroll
-            for (int i = 0; i < 16; ++i) s3[64 * j * P + i] = w[i];
-            if (j == 0) bg.template tick<0>(); else bg.template tick<1>();
-        }
+        for (int n = 0; n < 32; ++n) s[4 * n] = v[n];
     }
     pty_cta_sync();
-    {   // phase 2' (L2): conj twiddle, inverse radix-8 over k1x, (My), inverse radix-4 over k2y, conj twiddle
-        float2* s2 = c.slot2();
-        const int k1y = c.tid >> 4;
-        const float2* tx = c.twx + (c.tid & 15);
+    {   // thread (g, x = cc) takes ky = 8 g + i + 32 k2 into v[8 k2 + i]
+        const float2* s = c.X + (8 * g) * P + cc;
 #pragma unroll
-        for (int k2y = 0; k2y < 4; ++k2y) {
-            float2 w[8];
-            w[0] = s2[k2y * P];
-#pragma unroll
-            for (int k1 = 1; k1 < 8; ++k1) w[k1] = cmulc(tx[16 * k1], s2[k2y * P + 17 * k1]);
-            RegFFT<8, DIR>::run(w);
-            if (MY != 0) {
-                float2 m = c.My[k1y + 32 * k2y];
-                if (MY < 0) m.y = -m.y;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) w[i] = cmul(w[i], m);
-            }
-#pragma unroll
-            for (int i = 0; i < 8; ++i) v[8 * k2y + i] = w[i];
-            if (k2y == 1) bg.template tick<2>();
+        for (int i = 0; i < 8; ++i) {        // in the order the butterflies consume them
+            v[i] = s[i * P];
+            v[8 + i] = s[(i + 32) * P];
+            v[16 + i] = s[(i + 64) * P];
+            v[24 + i] = s[(i + 96) * P];
         }
-        bg.template tick<3>();
-        const float2* ty = c.twy + 4 * k1y;
-        const float2 wy1 = ty[1], wy2 = ty[2], wy3 = ty[3];
-#pragma unroll
-        for (int n1x = 0; n1x < 8; ++n1x) {
-            float2 a0 = v[n1x], a1 = v[8 + n1x], a2 = v[16 + n1x], a3 = v[24 + n1x];
-            bfly4<DIR>(a0, a1, a2, a3);                                              // -> q = 0..3
-            s2[17 * n1x] = a0;
-            s2[P + 17 * n1x] = cmulc(wy1, a1);
-            s2[2 * P + 17 * n1x] = cmulc(wy2, a2);
-            s2[3 * P + 17 * n1x] = cmulc(wy3, a3);
-            if (n1x == 3) bg.template tick<4>();
-        }
-        bg.template tick<5>();
     }
-    pty_cta_sync();
-    {   // phase 1' (L1): inverse radix-32 over k1y
-        const float2* s1 = c.slot1();
-#pragma unroll
-        for (int n2 = 0; n2 < 8; ++n2) {         // in the order the first butterflies consume them
-            v[n2] = s1[4 * n2 * P];
-            v[8 + n2] = s1[4 * (8 + n2) * P];
-            v[16 + n2] = s1[4 * (16 + n2) * P];
-            v[24 + n2] = s1[4 * (24 + n2) * P];
-        }
-        bg.template tick<6>();
-        fft32<DIR>(v);
-        bg.template tick<7>();
-    }
+    // y axis
+    f128_radix4_inv<4, 5>(c, v, bg);
+    f128_tmem_exchange<false>(c, v);
+    fft32<+1, 6>(v, bg);
+    bg.template tick<7>();
 }
-template <int MY> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_inverse<MY>(c, v, bg); }
+
+PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_forward(c, v, bg); }
+PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_inverse(c, v, bg); }
 
 }  // namespace pty

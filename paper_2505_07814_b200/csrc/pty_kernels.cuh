@@ -36,6 +36,7 @@ struct KArgs {
     float2* ws_hat;            // [B][M][Nz-1][N][N] spectrum of psi_{s+1} (times 1/N), optional
     float2* GP_hat;            // [M][N][N]   sum_b conj(E_b) F[g_psi0]
     float* dsum;               // [B][4]      sum_k D (k_py, k_px, |k_p|^2)
+    float* seed_w;             // [B][32][512] seed weights 2 (1 - a / sqrt(I)) / N in thread order (N = 128 register path)
     int* flags;                // sticky device flags (bit 0: a crop was clamped)
     float2* g_object;          // [Nz][H][W]
     float* g_pos;              // [B][2]

@@ -1,11 +1,13 @@
 // pty_kernels128.cuh -- forward and adjoint bodies for N = 128 on the register-resident FFT
 // (pty_fft128.cuh): one CTA of 512 threads per (position b, probe mode m); the wave stays in
 // registers through the whole slice chain, every pointwise step of the method runs on registers in
-// layout L1 (real space: rows y = 4 n1 + q of column x) or L3 (k space: ky(j), k1x + 8 k2x; pty_fft128.cuh).
+// layout R (real space: rows y = 4 n1 + q of column x = c) or layout K (k space: row ky = c,
+// columns kx = 8 g + i + 32 k2 in register 8 k2 + i).
 //
-// Workspace layouts: psi (incident waves) natural [y][x]; Psi (far field) and the kept spectra in
-// "thread order" [register][tid] (private to these kernels, perfectly coalesced).
-// Same scaling conventions as pty_kernels.cuh (Ex carries 1/N, Mx carries 1/N^2).
+// Workspace layouts: psi (incident waves) natural [y][x]; every k-space array private to these
+// kernels (P^, Psi, the kept spectra, the seed weights, G^_P) in "thread order" [register][tid], which
+// is perfectly coalesced in layout K.  Same scaling conventions as pty_kernels.cuh (Ex carries 1/N,
+// Mx carries 1/N^2).
 #pragma once
 #include "pty_fft128.cuh"
 #include "pty_kernels.cuh"
@@ -26,7 +28,7 @@ PTY_DEV void block_accumulate128(const Cta128& c, int slot, float v) {
 // ------------------------------------------------------------------------------ background fetches
 // Fetch 32 float2 per thread (rows n1 = 0..31 at stride `stride` float2 from p) into tensor memory
 // columns [tm, tm + 64), four rows per tick: tick K parks the rows fetched by tick K - 1 and issues the
-// loads of rows 4 K .. 4 K + 3.  The rows of the last tick stay in `buf` (use take<7>()).
+// loads of rows 4 K .. 4 K + 3.  The rows of the last tick stay in `buf` (take<7>).
 template <bool STREAM> struct Fetch32 {
     const float2* p;
     size_t stride;
@@ -56,30 +58,23 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     setup128(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)b * A.M + m;
-    const int q = c.q(), x = c.x(), k1x = c.k1x();
+    const int g = c.g(), cc = c.cc();
     float2 v[32];
     // a3: the object rows of slice s are fetched during the inverse transform that precedes their use
     Fetch32<false> fo;
-    fo.p = A.object + ((size_t)ry + q) * A.W + rx + x;
+    fo.p = A.object + ((size_t)ry + g) * A.W + rx + cc;
     fo.stride = (size_t)4 * A.W;
-    fo.tm = c.tm;
-    {   // a2: psi_0 = F^-1[E . P^]   (L3 -> L1)
-        const float2* Ph = A.probe_hat + (size_t)m * NN;
+    fo.tm = c.tm_s();
+    {   // a2: psi_0 = F^-1[E . P^]   (K -> R)
+        const float2* Ph = A.probe_hat + (size_t)m * NN + c.tid;
+        const float2 ey = c.Ey[cc];
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const int ky = c.ky(j);
-            const float2 ey = c.Ey[ky];
-#pragma unroll
-            for (int k2 = 0; k2 < 16; ++k2) {
-                const int kx = k1x + 8 * k2;
-                v[16 * j + k2] = cmul(cmul(ldg2(Ph + ky * N + kx), ey), c.Ex[kx]);
-            }
-        }
-        f128_inverse<0>(c, v, fo);
+        for (int r = 0; r < 32; ++r) v[r] = cmul(cmul(ldg2(Ph + r * F128::NT), ey), c.Ex[c.kx(r)]);
+        f128_inverse(c, v, fo);
     }
     for (int s = 0; s < A.Nz; ++s) {
-        {   // a3 + a4 (L1): keep psi_{s-1}, phi_s = O_b[s] psi_{s-1}
-            float2* save = A.ws_psi + (bm * A.Nz + s) * NN + q * N + x;
+        {   // a3 + a4 (R): keep psi_{s-1}, phi_s = O_b[s] psi_{s-1}
+            float2* save = A.ws_psi + (bm * A.Nz + s) * NN + g * N + cc;
             tmem_wait_st();
 #define PTY_OBJ_CHUNK(K)                                                   \
             {                                                              \
@@ -90,31 +85,41 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
                     v[4 * K + i] = cmul(v[4 * K + i], o[i]);               \
                 }                                                          \
             }
-            PTY_OBJ_CHUNK(7) PTY_OBJ_CHUNK(0) PTY_OBJ_CHUNK(1) PTY_OBJ_CHUNK(2)
-            PTY_OBJ_CHUNK(3) PTY_OBJ_CHUNK(4) PTY_OBJ_CHUNK(5) PTY_OBJ_CHUNK(6)
+            PTY_OBJ_CHUNK(0) PTY_OBJ_CHUNK(1) PTY_OBJ_CHUNK(2) PTY_OBJ_CHUNK(3)
+            PTY_OBJ_CHUNK(4) PTY_OBJ_CHUNK(5) PTY_OBJ_CHUNK(6) PTY_OBJ_CHUNK(7)
 #undef PTY_OBJ_CHUNK
             fo.p += (size_t)A.H * A.W;
         }
         f128_forward(c, v);
         if (s == A.Nz - 1) break;
-        {   // a4 (L3): k_x factor of the propagator (k_y factor inside the inverse); keep the spectrum
+        {   // a4 (K): propagator M = My[ky] Mx[kx] (/N^2); keep the spectrum F[psi_s]
             float2* hat = A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + s) * NN + c.tid : nullptr;
+            const float2 my = c.My[cc];
 #pragma unroll
             for (int r = 0; r < 32; ++r) {
-                v[r] = cmul(v[r], c.Mx[k1x + 8 * (r & 15)]);
+                v[r] = cmul(v[r], cmul(my, c.Mx[c.kx(r)]));
                 if (hat) st_stream2(hat + r * F128::NT, v[r]);
             }
         }
-        f128_inverse<+1>(c, v, fo);
+        f128_inverse(c, v, fo);
     }
-    // a5 (L3): Psi = F[phi_Nz] / N, I += |Psi|^2
+    // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2 (transposed through X so that the reductions into the
+    // natural [ky][kx] array are coalesced)
     float2* Psi = A.ws_Psi + bm * NN + c.tid;
-    float* Ib = A.I + (size_t)b * NN;
+    float* Xf = reinterpret_cast<float*>(c.X);
+    pty_cta_sync();                                   // every thread is done with the last transpose
 #pragma unroll
     for (int r = 0; r < 32; ++r) {
         const float2 p = cscale(v[r], 1.0f / N);
         st_stream2(Psi + r * F128::NT, p);
-        red_add(Ib + c.ky(r >> 4) * N + k1x + 8 * (r & 15), p.x * p.x + p.y * p.y);
+        Xf[cc * F128::P + c.kx(r)] = p.x * p.x + p.y * p.y;
+    }
+    pty_cta_sync();
+    float* Ib = A.I + (size_t)b * NN;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+        const int idx = j * F128::NT + c.tid;
+        red_add(Ib + idx, Xf[(idx >> 7) * F128::P + (idx & 127)]);
     }
 }
 
@@ -126,37 +131,31 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
     setup128(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)b * A.M + m;
-    const int q = c.q(), x = c.x(), k1x = c.k1x();
+    const int g = c.g(), cc = c.cc();
     float2 v[32];
-    {   // a7, a8 (L3): g_Psi = 2 (1 - a / sqrt(I)) Psi, g_phi = F^-1[g_Psi]
+    {   // a7, a8 (K): g_Psi = w Psi with the seed weights w = 2 (1 - a / sqrt(I)) / N, g_phi = F^-1[g_Psi]
         const float2* Psi = A.ws_Psi + bm * NN + c.tid;
-        const float* Ib = A.I + (size_t)b * NN;
-        const float* ab = A.meas + (size_t)b * NN;
+        const float* Wt = A.seed_w + (size_t)b * NN + c.tid;
 #pragma unroll
         for (int h = 0; h < 32; h += 8) {
-            float iv[8], av[8];
+            float wv[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const int r = h + i, idx = c.ky(r >> 4) * N + k1x + 8 * (r & 15);
-                v[r] = ld_stream2(Psi + r * F128::NT);
-                iv[i] = ldg1(Ib + idx);
-                av[i] = ldg1(ab + idx);
+                v[h + i] = ld_stream2(Psi + (h + i) * F128::NT);
+                wv[i] = ldg1(Wt + (h + i) * F128::NT);
             }
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const float w = iv[i] > 1e-30f ? 2.0f * (1.0f - av[i] * rsqrt_f(iv[i])) * (1.0f / N) : 0.f;
-                v[h + i] = cscale(v[h + i], w);
-            }
+            for (int i = 0; i < 8; ++i) v[h + i] = cscale(v[h + i], wv[i]);
         }
-        f128_inverse<0>(c, v);
+        f128_inverse(c, v);
     }
     float acc_ky = 0.f, acc_kx = 0.f, acc_k2 = 0.f;
     for (int s = A.Nz - 1; s >= 0; --s) {
-        {   // a9, a10 (L1): g_object patch += conj(psi_{s-1}) g;  g <- conj(O_b[s]) g
-            const size_t off = ((size_t)s * A.H + ry + q) * A.W + rx + x;
+        {   // a9, a10 (R): g_object patch += conj(psi_{s-1}) g;  g <- conj(O_b[s]) g
+            const size_t off = ((size_t)s * A.H + ry + g) * A.W + rx + cc;
             const float2* obj = A.object + off;
             float2* gobj = A.g_object + off;
-            const float2* psi = A.ws_psi + (bm * A.Nz + s) * NN + q * N + x;
+            const float2* psi = A.ws_psi + (bm * A.Nz + s) * NN + g * N + cc;
 #pragma unroll
             for (int h = 0; h < 32; h += 8) {
                 float2 ps[8], o[8];
@@ -174,48 +173,41 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
         }
         f128_forward(c, v);
         if (s == 0) break;
-        {   // a9, a13 (L3): D-sums against the kept spectrum, then conj(Mx) (conj(My) inside the inverse)
+        {   // a9, a13 (K): D-sums against the kept spectrum, then conj(M)
+            const float2 my = c.My[cc];
             if (A.save_hat) {
                 const float2* hat = A.ws_hat + (bm * (A.Nz - 1) + (s - 1)) * NN + c.tid;
+                const float kyf = kp_of<N>(cc);
 #pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const int ky = c.ky(j);
-                    const float2 my = c.My[ky];
-                    const float kyf = kp_of<N>(ky);
-#pragma unroll
-                    for (int k2 = 0; k2 < 16; ++k2) {
-                        const int r = 16 * j + k2;
-                        const float2 hs = cmul(my, ld_stream2(hat + r * F128::NT));
-                        const float d = hs.x * v[r].y - hs.y * v[r].x;          // Im(conj(psi^) g^)
-                        const float kxf = kp_of<N>(k1x + 8 * k2);
-                        acc_ky += d * kyf;
-                        acc_kx += d * kxf;
-                        acc_k2 += d * (kyf * kyf + kxf * kxf);
-                    }
+                for (int r = 0; r < 32; ++r) {
+                    const float2 hs = ld_stream2(hat + r * F128::NT);
+                    const float d = hs.x * v[r].y - hs.y * v[r].x;          // Im(conj(psi^) g^)
+                    const float kxf = kp_of<N>(c.kx(r));
+                    acc_ky += d * kyf;
+                    acc_kx += d * kxf;
+                    acc_k2 += d * (kyf * kyf + kxf * kxf);
                 }
             }
 #pragma unroll
-            for (int r = 0; r < 32; ++r) v[r] = cmulc(c.Mx[k1x + 8 * (r & 15)], v[r]);
+            for (int r = 0; r < 32; ++r) v[r] = cmulc(cmul(my, c.Mx[c.kx(r)]), v[r]);
         }
-        f128_inverse<-1>(c, v);
+        f128_inverse(c, v);
     }
-    // a11, a12 (L3): g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
-    const float2* Ph = A.probe_hat + (size_t)m * NN;
-    float2* GP = A.GP_hat + (size_t)m * NN;
+    // a11, a12 (K): g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
+    const float2* Ph = A.probe_hat + (size_t)m * NN + c.tid;
+    float2* GP = A.GP_hat + (size_t)m * NN + c.tid;
     float accy = 0.f, accx = 0.f;
+    {
+        const float2 ey = c.Ey[cc];
+        const float kyf = kp_of<N>(cc);
 #pragma unroll
-    for (int j = 0; j < 2; ++j) {
-        const int ky = c.ky(j);
-        const float2 ey = c.Ey[ky];
-        const float kyf = kp_of<N>(ky);
-#pragma unroll
-        for (int k2 = 0; k2 < 16; ++k2) {
-            const int kx = k1x + 8 * k2;
-            const float2 g = v[16 * j + k2];
+        for (int r = 0; r < 32; ++r) {
+            const int kx = c.kx(r);
+            const float2 gg = v[r];
             const float2 e = cmul(ey, c.Ex[kx]);                     // E / N
-            red_add2(GP + ky * N + kx, cmulc(e, g));
-            const float2 ep = cmul(e, ldg2(Ph + ky * N + kx));
-            const float t = g.x * ep.y - g.y * ep.x;                 // Im(conj(g^_0) E P^)
+            red_add2(GP + r * F128::NT, cmulc(e, gg));
+            const float2 ep = cmul(e, ldg2(Ph + r * F128::NT));
+            const float t = gg.x * ep.y - gg.y * ep.x;               // Im(conj(g^_0) E P^)
             accy += kyf * t;
             accx += kp_of<N>(kx) * t;
         }
@@ -239,6 +231,41 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
             red_add(A.dsum + 4 * b + 1, c.red[3]);
             red_add(A.dsum + 4 * b + 2, c.red[4]);
         }
+    }
+}
+
+// ------------------------------------------------------------------------------ a0 / a11 helpers
+// P^_t[m] = F[P[m]] / N in thread order (one CTA per mode)
+PTY_DEV void probe_hat_body128(const float2* probe, float2* probe_hat_t, const Cta128& c, int m) {
+    constexpr int N = 128;
+    f128_fill_twiddles(c);
+    pty_cta_sync();
+    const float2* src = probe + (size_t)m * N * N + c.g() * N + c.cc();
+    float2 v[32];
+#pragma unroll
+    for (int n = 0; n < 32; ++n) v[n] = ldg2(src + 4 * n * N);
+    f128_forward(c, v);
+    float2* dst = probe_hat_t + (size_t)m * N * N + c.tid;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) dst[r * F128::NT] = cscale(v[r], 1.0f / N);
+}
+
+// g_probe[m] (+)= F^-1[G^_P_t[m]] / N (one CTA per mode)
+PTY_DEV void probe_grad_body128(const float2* GP_t, float2* g_probe, int accumulate, const Cta128& c, int m) {
+    constexpr int N = 128;
+    f128_fill_twiddles(c);
+    pty_cta_sync();
+    const float2* src = GP_t + (size_t)m * N * N + c.tid;
+    float2 v[32];
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = src[r * F128::NT];
+    f128_inverse(c, v);
+    float2* dst = g_probe + (size_t)m * N * N + c.g() * N + c.cc();
+#pragma unroll
+    for (int n = 0; n < 32; ++n) {
+        float2 o = cscale(v[n], 1.0f / N);
+        if (accumulate) o = cadd(o, dst[4 * n * N]);
+        dst[4 * n * N] = o;
     }
 }
 

@@ -61,17 +61,15 @@ __device__ __forceinline__ Cta128 make_cta128(unsigned char* smem) {
     c.tid = threadIdx.x;
     c.X = reinterpret_cast<float2*>(smem);
     float2* tab = reinterpret_cast<float2*>(smem + F128::xch_bytes);
-    c.twy = tab; c.twx = tab + 128; c.Ey = tab + 256; c.Ex = tab + 384; c.My = tab + 512; c.Mx = tab + 640;
-    c.red = reinterpret_cast<float*>(tab + 768);
-    // tensor memory: all 512 columns, allocated by warp 0; thread block = lane quarter (warp % 4),
-    // columns [128 (warp / 4), + 128)
+    c.twg = tab; c.Ey = tab + 128; c.Ex = tab + 256; c.My = tab + 384; c.Mx = tab + 512;
+    c.red = reinterpret_cast<float*>(tab + 640);
+    // tensor memory: all 512 columns, allocated by warp 0; thread (g, c) owns lane c, columns [128 g, +128)
     unsigned* tbase = reinterpret_cast<unsigned*>(c.red + 64);
     if ((threadIdx.x >> 5) == 0) tmem_alloc512(tbase);
     tmem_fence_before_sync();
     __syncthreads();
     tmem_fence_after_sync();
-    const unsigned w = threadIdx.x >> 5;
-    c.tm = *tbase + ((32u * (w & 3u)) << 16) + 128u * (w >> 2);
+    c.tmq = *tbase + ((32u * ((threadIdx.x >> 5) & 3u)) << 16);
     return c;
 }
 
@@ -79,7 +77,7 @@ __device__ __forceinline__ void release_cta128(unsigned char* smem) {
     tmem_fence_before_sync();
     __syncthreads();
     float2* tab = reinterpret_cast<float2*>(smem + F128::xch_bytes);
-    if ((threadIdx.x >> 5) == 0) tmem_dealloc512(*reinterpret_cast<unsigned*>(reinterpret_cast<float*>(tab + 768) + 64));
+    if ((threadIdx.x >> 5) == 0) tmem_dealloc512(*reinterpret_cast<unsigned*>(reinterpret_cast<float*>(tab + 640) + 64));
 }
 
 __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128_kernel(const KArgs A) {
@@ -92,6 +90,63 @@ __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128_kernel(const KArgs A) 
     extern __shared__ __align__(16) unsigned char smem[];
     bwd_body128(A, make_cta128(smem), blockIdx.x);
     release_cta128(smem);
+}
+
+// a0: P^ = F[P] / N in thread order; a11: g_probe = F^-1[G^_P] / N (one CTA per mode)
+__global__ void __launch_bounds__(F128::NT, 1) pty_probe_hat128_kernel(const float2* probe, float2* probe_hat_t) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    probe_hat_body128(probe, probe_hat_t, make_cta128(smem), blockIdx.x);
+    release_cta128(smem);
+}
+__global__ void __launch_bounds__(F128::NT, 1) pty_probe_grad128_kernel(const float2* GP_t, float2* g_probe, int accumulate) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    probe_grad_body128(GP_t, g_probe, accumulate, make_cta128(smem), blockIdx.x);
+    release_cta128(smem);
+}
+
+// a6 + a7 for the N = 128 register path: L_b = sum_k (sqrt(I_b) - a_b)^2 and the seed weights
+// w = 2 (1 - a / sqrt(I)) / N (0 where I = 0, reading R14) written in the adjoint kernel's thread
+// order [register r = 8 (kx >> 5) + (kx & 7)][tid = 128 ((kx >> 3) & 3) + ky].  One block of 256 threads
+// per position; 32-row tiles are transposed through shared memory so that both sides are coalesced.
+__global__ void __launch_bounds__(256) pty_loss_seed128_kernel(const float* __restrict__ I, const float* __restrict__ a,
+                                                              double* loss, float* loss_per_pos, float* __restrict__ seed_w) {
+    constexpr int N = 128;
+    __shared__ float tile[32][N + 1];
+    __shared__ double part[8];
+    const int b = blockIdx.x, t = threadIdx.x;
+    const float* Ib = I + (size_t)b * N * N;
+    const float* ab = a + (size_t)b * N * N;
+    float* Wb = seed_w + (size_t)b * N * N;
+    float acc = 0.f;
+    for (int ky0 = 0; ky0 < N; ky0 += 32) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int idx = j * 256 + t, row = idx >> 7, kx = idx & 127;
+            const float iv = __ldg(Ib + (ky0 + row) * N + kx), av = __ldg(ab + (ky0 + row) * N + kx);
+            const float d = sqrtf(iv) - av;
+            acc += d * d;
+            tile[row][kx] = iv > 1e-30f ? 2.0f * (1.0f - av * rsqrtf(iv)) * (1.0f / N) : 0.f;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int idx = j * 256 + t, row = idx & 31, kx = idx >> 5;
+            const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3;
+            Wb[r * 512 + 128 * g + ky0 + row] = tile[row][kx];
+        }
+        __syncthreads();
+    }
+    double dacc = (double)acc;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dacc += __shfl_xor_sync(0xffffffffu, dacc, o);
+    if ((t & 31) == 0) part[t >> 5] = dacc;
+    __syncthreads();
+    if (t == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += part[w];
+        if (loss_per_pos) loss_per_pos[b] = (float)s;
+        atomicAdd(loss, s);
+    }
 }
 
 template <class SH, int DIR>
@@ -212,7 +267,7 @@ namespace {
 thread_local std::string g_create_error;
 
 struct Layout {
-    size_t probe_hat, prop, I, ws_psi, ws_Psi, ws_hat, GP_hat, dsum, scalars;
+    size_t probe_hat, prop, I, ws_psi, ws_Psi, ws_hat, GP_hat, dsum, seed_w, scalars;
     size_t g_object, g_probe, g_pos, g_tilt;               // PTY_FLAG_STEP / PTY_FLAG_HOST
     size_t h_object, h_probe, h_pos, h_tilt, h_meas;       // PTY_FLAG_HOST staging
     size_t total;
@@ -245,6 +300,7 @@ Layout make_layout(const pty_dims& d) {
     L.ws_hat = take(save_hat_of(d) ? B * M * (Nz - 1) * NN * 8 : 0);
     L.GP_hat = take(M * NN * 8);
     L.dsum = take(B * 4 * 4);
+    L.seed_w = take(d.N == 128 ? B * NN * 4 : 0);
     L.scalars = take(256);
     const bool grads = d.flags & (PTY_FLAG_STEP | PTY_FLAG_HOST);
     const size_t obj = Nz * (size_t)d.H * d.W * 8;
@@ -401,6 +457,7 @@ KArgs make_args(const pty_plan* p, const void* object, const float* positions, c
     A.ws_hat = A.save_hat ? p->at<float2>(p->L.ws_hat) : nullptr;
     A.GP_hat = p->at<float2>(p->L.GP_hat);
     A.dsum = p->at<float>(p->L.dsum);
+    A.seed_w = p->at<float>(p->L.seed_w);
     A.flags = p->d_flags();
     return A;
 }
@@ -425,15 +482,21 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
     if (B == 0) return PTY_OK;
     KArgs A = make_args(p, object, positions, tilt, meas, B);
     // a0: probe spectrum (unitary) and propagator factors
-    PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fft2<Shape<64>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
-                               launch_fft2<Shape<128>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
-                               launch_fft2<Shape<256>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st)));
+    if (d.N == 128 && p->reg128)
+        PTY_CUDA(p, launch(p, pty_probe_hat128_kernel, d.M, F128::NT, F128::smem_bytes, 1, st, (const float2*)probe, p->at<float2>(p->L.probe_hat)));
+    else
+        PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fft2<Shape<64>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
+                                   launch_fft2<Shape<128>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
+                                   launch_fft2<Shape<256>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st)));
     if (d.tilt_mode != 2)
         PTY_CUDA(p, launch(p, pty_prop_table_kernel, (d.N + 127) / 128, 128, 0, 1, st, (int)d.N, d.dz, d.lambda, d.dx,
                            d.tilt_mode == 1 ? tilt : (const float*)nullptr, p->at<float2>(p->L.prop), p->at<float2>(p->L.prop) + d.N));
     PTY_CUDA(p, cudaMemsetAsync(A.I, 0, (size_t)B * NN * sizeof(float), st));
     PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fwd<Shape<64>>(p, A, st), launch_fwd<Shape<128>>(p, A, st), launch_fwd<Shape<256>>(p, A, st)));
-    PTY_CUDA(p, launch(p, pty_loss_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)NN, loss, loss_per_pos));
+    if (d.N == 128 && p->reg128)
+        PTY_CUDA(p, launch(p, pty_loss_seed128_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w));
+    else
+        PTY_CUDA(p, launch(p, pty_loss_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)NN, loss, loss_per_pos));
     if (intensity)
         PTY_CUDA(p, cudaMemcpyAsync(intensity, A.I, (size_t)B * NN * sizeof(float), cudaMemcpyDeviceToDevice, st));
     p->fwd_valid = true;
@@ -461,7 +524,9 @@ int run_backward(pty_plan* p, const void* object, const float* positions, const 
     if (A.save_hat && B) PTY_CUDA(p, cudaMemsetAsync(A.dsum, 0, (size_t)B * 4 * sizeof(float), st));
     if (B)
         PTY_CUDA(p, PTY_DISPATCH_N(p, launch_bwd<Shape<64>>(p, A, st), launch_bwd<Shape<128>>(p, A, st), launch_bwd<Shape<256>>(p, A, st)));
-    if (want_probe)
+    if (want_probe && d.N == 128 && p->reg128)
+        PTY_CUDA(p, launch(p, pty_probe_grad128_kernel, d.M, F128::NT, F128::smem_bytes, 1, st, (const float2*)A.GP_hat, (float2*)g_probe, (int)accumulate));
+    else if (want_probe)
         PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fft2<Shape<64>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st),
                                    launch_fft2<Shape<128>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st),
                                    launch_fft2<Shape<256>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st)));
@@ -538,6 +603,10 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
         e = cudaFuncSetAttribute(pty_fwd128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_bwd128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_probe_hat128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_probe_grad128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
     }
     if (e == cudaSuccess) e = cudaMemset(p->ws + L.scalars, 0, 256);
     if (e != cudaSuccess) {
