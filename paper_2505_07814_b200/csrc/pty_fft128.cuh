@@ -73,14 +73,16 @@ template <int J, int DIR> PTY_DEV float2 mul_w32(float2 a) {
     else return mul_cs<DIR>(a, c, s);
 }
 
-// Background work interleaved with a transform: the transforms call bg.tick<K>() at 8 points spread
-// over their arithmetic (K = 0..7 in program order); the kernel bodies use the ticks to fetch the
-// global data of the NEXT pointwise step in small chunks and park it in tensor memory.
+// Background work interleaved with a transform: the transforms call bg.tick<K>() at points spread over
+// their arithmetic (K = 0, 1, ... in program order); the kernel bodies use the ticks to fetch the global
+// data of the NEXT pointwise step in small chunks and park it in tensor memory.  The inverse transform
+// has 9 ticks (0..8) before its last TMEM exchange and 6 ticks of a second functor (0..5) after it, when
+// the exchange block is free and can serve as a second staging buffer.
 struct NoBg { template <int K> PTY_DEV void tick() {} };
 
 // 32-point DFT in registers, natural order in and out.  n = 8 n1 + n2, k = k1 + 4 k2.
-// One tick (TK) between its two stages.
-template <int DIR, int TK, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg) {
+// Four ticks TB .. TB + 3: after the first stage and after each of the first three radix-8 groups.
+template <int DIR, int TB, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg) {
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) bfly4<DIR>(v[n2], v[8 + n2], v[16 + n2], v[24 + n2]);   // -> v[8 k1 + n2]
 #define PTY_TW(K1, N2) v[8 * K1 + N2] = mul_w32<K1 * N2, DIR>(v[8 * K1 + N2]);
@@ -88,7 +90,7 @@ template <int DIR, int TK, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg)
     PTY_TW(2, 1) PTY_TW(2, 2) PTY_TW(2, 3) PTY_TW(2, 4) PTY_TW(2, 5) PTY_TW(2, 6) PTY_TW(2, 7)
     PTY_TW(3, 1) PTY_TW(3, 2) PTY_TW(3, 3) PTY_TW(3, 4) PTY_TW(3, 5) PTY_TW(3, 6) PTY_TW(3, 7)
 #undef PTY_TW
-    bg.template tick<TK>();
+    bg.template tick<TB>();
     float2 o[32];
 #pragma unroll
     for (int k1 = 0; k1 < 4; ++k1) {
@@ -98,6 +100,9 @@ template <int DIR, int TK, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg)
         RegFFT<8, DIR>::run(w);
 #pragma unroll
         for (int k2 = 0; k2 < 8; ++k2) o[k1 + 4 * k2] = w[k2];
+        if (k1 == 0) bg.template tick<TB + 1>();
+        if (k1 == 1) bg.template tick<TB + 2>();
+        if (k1 == 2) bg.template tick<TB + 3>();
     }
 #pragma unroll
     for (int k = 0; k < 32; ++k) v[k] = o[k];
@@ -120,7 +125,9 @@ PTY_DEV void f128_fill_twiddles(const Cta128& c) {
 PTY_DEV void subpartition_sync(int tid) {      // the 4 warps {w, w+4, w+8, w+12} of one SM sub-partition
     asm volatile("bar.sync %0, 128;" ::"r"(1 + ((tid >> 5) & 3)) : "memory");
 }
-template <bool WAR> PTY_DEV void f128_tmem_exchange(const Cta128& c, float2 (&v)[32]) {
+// FREE: also wait, after the reads, until the partners have read this thread's block, so that the block
+// can be reused as a staging buffer (the next exchange then needs no WAR wait).
+template <bool WAR, bool FREE> PTY_DEV void f128_tmem_exchange(const Cta128& c, float2 (&v)[32]) {
     if (WAR) {
         tmem_fence_before_sync();
         subpartition_sync(c.tid);
@@ -137,6 +144,11 @@ template <bool WAR> PTY_DEV void f128_tmem_exchange(const Cta128& c, float2 (&v)
 #pragma unroll
     for (int g2 = 0; g2 < 4; ++g2) tmem_ld8(c.tmq + 128u * g2 + col, v, 8 * g2);
     tmem_wait_ld();
+    if (FREE) {
+        tmem_fence_before_sync();
+        subpartition_sync(c.tid);
+        tmem_fence_after_sync();
+    }
 }
 
 // ------------------------------------------------------------------------------ radix-4 stage (c)
@@ -175,14 +187,16 @@ template <int T0, int T1, class BG> PTY_DEV void f128_radix4_inv(const Cta128& c
 
 // ------------------------------------------------------------------------------ forward, R -> K
 // in: v[n1] = a[4 n1 + q][x];  out: v[8 k2 + i] = A[ky = c][kx = 8 g + i + 32 k2]  (unscaled).
-template <class BG> PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32], BG& bg) {
+// WAR0: the first exchange must wait for the partners' reads of the previous exchange (false when the
+// preceding inverse ended with a FREE exchange).  14 ticks.
+template <bool WAR0, class BG> PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32], BG& bg) {
     constexpr int P = F128::P;
     const int g = c.g(), cc = c.cc();
     // y axis
     bg.template tick<0>();
     fft32<-1, 1>(v, bg);
-    f128_tmem_exchange<true>(c, v);
-    f128_radix4_fwd<2, 3>(c, v, bg);
+    f128_tmem_exchange<WAR0, false>(c, v);
+    f128_radix4_fwd<5, 6>(c, v, bg);
     {   // S: thread (g, x = cc) holds ky = 8 g + i + 32 k2 in v[8 k2 + i]
         float2* s = c.X + (8 * g) * P + cc;
 #pragma unroll
@@ -200,22 +214,22 @@ template <class BG> PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32], 
         }
     }
     // x axis
-    bg.template tick<4>();
-    fft32<-1, 5>(v, bg);
-    f128_tmem_exchange<false>(c, v);
-    f128_radix4_fwd<6, 7>(c, v, bg);
+    bg.template tick<7>();
+    fft32<-1, 8>(v, bg);
+    f128_tmem_exchange<false, false>(c, v);
+    f128_radix4_fwd<12, 13>(c, v, bg);
 }
 
 // ------------------------------------------------------------------------------ inverse, K -> R
 // in: v[8 k2 + i] = A[ky = c][kx = 8 g + i + 32 k2];  out: v[n1] = a[4 n1 + q][x]  (unscaled: x N^2).
-template <class BG> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32], BG& bg) {
+template <bool FREE, class BG, class BG2> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32], BG& bg, BG2& bg2) {
     constexpr int P = F128::P;
     const int g = c.g(), cc = c.cc();
     // x axis
     f128_radix4_inv<0, 1>(c, v, bg);
-    f128_tmem_exchange<true>(c, v);
+    f128_tmem_exchange<true, false>(c, v);
     fft32<+1, 2>(v, bg);
-    bg.template tick<3>();
+    bg.template tick<6>();
     {   // S: thread (xq = g, ky = cc) holds x = 4 n1x + xq in v[n1x]
         float2* s = c.X + cc * P + g;
 #pragma unroll
@@ -233,13 +247,14 @@ template <class BG> PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32], 
         }
     }
     // y axis
-    f128_radix4_inv<4, 5>(c, v, bg);
-    f128_tmem_exchange<false>(c, v);
-    fft32<+1, 6>(v, bg);
-    bg.template tick<7>();
+    f128_radix4_inv<7, 8>(c, v, bg);
+    f128_tmem_exchange<false, FREE>(c, v);
+    bg2.template tick<0>();
+    fft32<+1, 1>(v, bg2);
+    bg2.template tick<5>();
 }
 
-PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_forward(c, v, bg); }
-PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_inverse(c, v, bg); }
+PTY_DEV void f128_forward(const Cta128& c, float2 (&v)[32]) { NoBg bg; f128_forward<true>(c, v, bg); }
+PTY_DEV void f128_inverse(const Cta128& c, float2 (&v)[32]) { NoBg bg, bg2; f128_inverse<false>(c, v, bg, bg2); }
 
 }  // namespace pty

@@ -26,28 +26,43 @@ PTY_DEV void block_accumulate128(const Cta128& c, int slot, float v) {
 }
 
 // ------------------------------------------------------------------------------ background fetches
-// Fetch 32 float2 per thread (rows n1 = 0..31 at stride `stride` float2 from p) into tensor memory
-// columns [tm, tm + 64), four rows per tick: tick K parks the rows fetched by tick K - 1 and issues the
-// loads of rows 4 K .. 4 K + 3.  The rows of the last tick stay in `buf` (take<7>).
+// Fetch 32 float2 per thread (rows n1 = 0..31 at stride `stride` float2 from p) into the tensor-memory
+// staging block, four rows per tick: tick K (0..7) issues the loads of rows 4 K .. 4 K + 3, tick K + 1
+// parks them.  Nine ticks: everything is parked before the inverse transform's last exchange.
 template <bool STREAM> struct Fetch32 {
     const float2* p;
     size_t stride;
     unsigned tm;
     float2 buf[4];
     template <int K> PTY_DEV void tick() {
-        if (K > 0) tmem_st4(tm + 8 * (K - 1), buf);
+        if (K > 0 && K <= 8) tmem_st4(tm + 8 * (K - 1), buf);
+        if (K < 8) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-            buf[i] = STREAM ? ld_stream2_pinned(p + (size_t)(4 * K + i) * stride) : ldg2_pinned(p + (size_t)(4 * K + i) * stride);
-    }
-    // rows 4 K .. 4 K + 3 (after the transform that ran the ticks; tmem_wait_st() once before the first)
-    template <int K> PTY_DEV void take(float2 (&o)[4]) {
-        if (K < 7) { tmem_ld4(tm + 8 * K, o); tmem_wait_ld(); }
-        else {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) o[i] = buf[i];
+            for (int i = 0; i < 4; ++i)
+                buf[i] = STREAM ? ld_stream2_pinned(p + (size_t)(4 * K + i) * stride) : ldg2_pinned(p + (size_t)(4 * K + i) * stride);
         }
     }
+    // rows 4 K .. 4 K + 3 (tmem_wait_st() once before the first take)
+    template <int K> PTY_DEV void take(float2 (&o)[4]) { tmem_ld4(tm + 8 * K, o); tmem_wait_ld(); }
+};
+
+// Fetch 32 float2 per thread into the EXCHANGE block while it is free (after a FREE exchange), eight rows
+// per tick of the last fft32 of the inverse transform: ticks 0..3 issue rows 8 J .. 8 J + 7, ticks 1, 2, 3
+// and 5 park them.
+struct Fetch32x8 {
+    const float2* p;
+    size_t stride;
+    unsigned tm;
+    float2 buf[8];
+    template <int J> PTY_DEV void tick() {
+        if (J >= 1 && J <= 3) tmem_st8r(tm + 16 * (J - 1), buf);
+        if (J == 5) tmem_st8r(tm + 48, buf);
+        if (J <= 3) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) buf[i] = ldg2_pinned(p + (size_t)(8 * J + i) * stride);
+        }
+    }
+    template <int J> PTY_DEV void take(float2 (&o)[8]) { tmem_ld8r(tm + 16 * J, o); tmem_wait_ld(); }
 };
 
 // ------------------------------------------------------------------------------ forward (a2-a5)
@@ -65,12 +80,13 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     fo.p = A.object + ((size_t)ry + g) * A.W + rx + cc;
     fo.stride = (size_t)4 * A.W;
     fo.tm = c.tm_s();
+    NoBg nobg;
     {   // a2: psi_0 = F^-1[E . P^]   (K -> R)
         const float2* Ph = A.probe_hat + (size_t)m * NN + c.tid;
         const float2 ey = c.Ey[cc];
 #pragma unroll
         for (int r = 0; r < 32; ++r) v[r] = cmul(cmul(ldg2(Ph + r * F128::NT), ey), c.Ex[c.kx(r)]);
-        f128_inverse(c, v, fo);
+        f128_inverse<false>(c, v, fo, nobg);
     }
     for (int s = 0; s < A.Nz; ++s) {
         {   // a3 + a4 (R): keep psi_{s-1}, phi_s = O_b[s] psi_{s-1}
@@ -101,7 +117,7 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
                 if (hat) st_stream2(hat + r * F128::NT, v[r]);
             }
         }
-        f128_inverse(c, v, fo);
+        f128_inverse<false>(c, v, fo, nobg);
     }
     // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2 (transposed through X so that the reductions into the
     // natural [ky][kx] array are coalesced)
@@ -133,6 +149,18 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
     const size_t bm = (size_t)b * A.M + m;
     const int g = c.g(), cc = c.cc();
     float2 v[32];
+    // a9: the saved waves psi_{s-1} and the object rows O_b[s] of slice s are fetched during the inverse
+    // transform that precedes their use: psi (HBM stream) over its 9 ticks into the staging block, the
+    // object rows over the last fft32 into the exchange block once it is free.
+    Fetch32<true> fp;
+    fp.p = A.ws_psi + (bm * A.Nz + (A.Nz - 1)) * NN + g * N + cc;
+    fp.stride = (size_t)4 * N;
+    fp.tm = c.tm_s();
+    Fetch32x8 fo;
+    fo.p = A.object + ((size_t)(A.Nz - 1) * A.H + ry + g) * A.W + rx + cc;
+    fo.stride = (size_t)4 * A.W;
+    fo.tm = c.tm_x();
+    NoBg nobg;
     {   // a7, a8 (K): g_Psi = w Psi with the seed weights w = 2 (1 - a / sqrt(I)) / N, g_phi = F^-1[g_Psi]
         const float2* Psi = A.ws_Psi + bm * NN + c.tid;
         const float* Wt = A.seed_w + (size_t)b * NN + c.tid;
@@ -147,31 +175,31 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[h + i] = cscale(v[h + i], wv[i]);
         }
-        f128_inverse(c, v);
+        f128_inverse<true>(c, v, fp, fo);
     }
     float acc_ky = 0.f, acc_kx = 0.f, acc_k2 = 0.f;
     for (int s = A.Nz - 1; s >= 0; --s) {
         {   // a9, a10 (R): g_object patch += conj(psi_{s-1}) g;  g <- conj(O_b[s]) g
-            const size_t off = ((size_t)s * A.H + ry + g) * A.W + rx + cc;
-            const float2* obj = A.object + off;
-            float2* gobj = A.g_object + off;
-            const float2* psi = A.ws_psi + (bm * A.Nz + s) * NN + g * N + cc;
-#pragma unroll
-            for (int h = 0; h < 32; h += 8) {
-                float2 ps[8], o[8];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    ps[i] = ld_stream2(psi + 4 * (h + i) * N);
-                    o[i] = ldg2(obj + (size_t)(4 * (h + i)) * A.W);
-                }
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    red_add2(gobj + (size_t)(4 * (h + i)) * A.W, cmulc(ps[i], v[h + i]));
-                    v[h + i] = cmulc(o[i], v[h + i]);
-                }
+            float2* gobj = A.g_object + ((size_t)s * A.H + ry + g) * A.W + rx + cc;
+            tmem_wait_st();
+#define PTY_BWD_CHUNK(J)                                                                              \
+            {                                                                                         \
+                float2 o[8], pa[4], pb[4];                                                            \
+                fo.template take<J>(o);                                                               \
+                fp.template take<2 * J>(pa);                                                          \
+                fp.template take<2 * J + 1>(pb);                                                      \
+                _Pragma("unroll") for (int i = 0; i < 8; ++i) {                                       \
+                    const float2 ps = i < 4 ? pa[i & 3] : pb[i & 3];                                  \
+                    red_add2(gobj + (size_t)(4 * (8 * J + i)) * A.W, cmulc(ps, v[8 * J + i]));       \
+                    v[8 * J + i] = cmulc(o[i], v[8 * J + i]);                                         \
+                }                                                                                     \
             }
+            PTY_BWD_CHUNK(0) PTY_BWD_CHUNK(1) PTY_BWD_CHUNK(2) PTY_BWD_CHUNK(3)
+#undef PTY_BWD_CHUNK
+            fp.p -= (size_t)N * N;
+            fo.p -= (size_t)A.H * A.W;
         }
-        f128_forward(c, v);
+        f128_forward<false>(c, v, nobg);
         if (s == 0) break;
         {   // a9, a13 (K): D-sums against the kept spectrum, then conj(M)
             const float2 my = c.My[cc];
@@ -191,7 +219,7 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
 #pragma unroll
             for (int r = 0; r < 32; ++r) v[r] = cmulc(cmul(my, c.Mx[c.kx(r)]), v[r]);
         }
-        f128_inverse(c, v);
+        f128_inverse<true>(c, v, fp, fo);
     }
     // a11, a12 (K): g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
     const float2* Ph = A.probe_hat + (size_t)m * NN + c.tid;

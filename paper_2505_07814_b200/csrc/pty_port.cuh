@@ -72,6 +72,19 @@ PTY_DEV void tmem_ld8(unsigned ta, float2 (&v)[32], int o) {
                    "=f"(v[o + 6].x), "=f"(v[o + 6].y), "=f"(v[o + 7].x), "=f"(v[o + 7].y)
                  : "r"(ta) : "memory");
 }
+PTY_DEV void tmem_st8r(unsigned ta, const float2 (&v)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                 ::"r"(ta), "f"(v[0].x), "f"(v[0].y), "f"(v[1].x), "f"(v[1].y), "f"(v[2].x), "f"(v[2].y),
+                   "f"(v[3].x), "f"(v[3].y), "f"(v[4].x), "f"(v[4].y), "f"(v[5].x), "f"(v[5].y),
+                   "f"(v[6].x), "f"(v[6].y), "f"(v[7].x), "f"(v[7].y) : "memory");
+}
+PTY_DEV void tmem_ld8r(unsigned ta, float2 (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=f"(v[0].x), "=f"(v[0].y), "=f"(v[1].x), "=f"(v[1].y), "=f"(v[2].x), "=f"(v[2].y),
+                   "=f"(v[3].x), "=f"(v[3].y), "=f"(v[4].x), "=f"(v[4].y), "=f"(v[5].x), "=f"(v[5].y),
+                   "=f"(v[6].x), "=f"(v[6].y), "=f"(v[7].x), "=f"(v[7].y)
+                 : "r"(ta) : "memory");
+}
 // global load that the compiler must leave where it is written (prefetch ticks)
 PTY_DEV float2 ldg2_pinned(const float2* p) {
     float2 v;
