@@ -20,12 +20,40 @@
 namespace pty {
 
 // ----------------------------------------------------------------------------- complex helpers
+// Packed FP32x2 arithmetic (FADD2 / FMUL2 / FFMA2 on sm_100a): a complex value is one 64-bit register
+// pair, and the operand modifiers of the packed instructions (half swap, per-half negate, scalar
+// broadcast) absorb the swaps and sign changes, so every complex operation below is one or two
+// instructions.  Same FP32 lane throughput as scalar code, half the issue slots (profiles/r01_microbench.md).
+#ifndef PTY_PK_ADD
+#define PTY_PK_ADD 1
+#endif
+#ifndef PTY_PK_MUL
+#define PTY_PK_MUL 0
+#endif
+#ifndef PTY_PK_CS
+#define PTY_PK_CS 1
+#endif
+#if PTY_PK_ADD
+PTY_DEV float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+PTY_DEV float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+#else
 PTY_DEV float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 PTY_DEV float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-PTY_DEV float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+#endif
+#if PTY_PK_MUL
+PTY_DEV float2 cmul(float2 a, float2 b) {
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(-b.y, b.y), __fmul2_rn(a, make_float2(b.x, b.x)));
+}
 // conj(a) * b
+PTY_DEV float2 cmulc(float2 a, float2 b) {
+    return __ffma2_rn(make_float2(b.y, b.x), make_float2(a.y, -a.y), __fmul2_rn(b, make_float2(a.x, a.x)));
+}
+PTY_DEV float2 cscale(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+#else
+PTY_DEV float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 PTY_DEV float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }
 PTY_DEV float2 cscale(float2 a, float s) { return make_float2(a.x * s, a.y * s); }
+#endif
 PTY_DEV float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
 
 // a * exp(DIR * i * pi/2): forward multiplies by -i, inverse by +i
@@ -34,8 +62,14 @@ template <int DIR> PTY_DEV float2 mul_qi(float2 a) {
 }
 // a * (c + i*DIR*s) with c, s the cos/sin of a positive angle
 template <int DIR> PTY_DEV float2 mul_cs(float2 a, float c, float s) {
+#if PTY_PK_CS
+    const float2 t = __fmul2_rn(a, make_float2(c, c));
+    return DIR < 0 ? __ffma2_rn(make_float2(a.y, a.x), make_float2(s, -s), t)
+                   : __ffma2_rn(make_float2(a.y, a.x), make_float2(-s, s), t);
+#else
     return DIR < 0 ? make_float2(a.x * c + a.y * s, a.y * c - a.x * s)
                    : make_float2(a.x * c - a.y * s, a.y * c + a.x * s);
+#endif
 }
 
 // ----------------------------------------------------------------------------- radix-4 / 8 / 16
