@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpty.so")
 SOURCES = ["pty_lib.cu"]
-HEADERS = ["pty_port.cuh", "pty_fft.cuh", "pty_kernels.cuh", "pty_fft128.cuh", "pty_kernels128.cuh", os.path.join("..", "..", "include", "pty.h")]
+HEADERS = ["pty_port.cuh", "pty_fft.cuh", "pty_kernels.cuh", "pty_fft128.cuh", "pty_kernels128.cuh", "pty_kernels128g2.cuh", os.path.join("..", "..", "include", "pty.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -4,11 +4,15 @@
 // layout R (real space: rows y = 4 n1 + q of column x = c) or layout K (k space: row ky = c,
 // columns kx = 8 g + i + 32 k2 in register 8 k2 + i).
 //
-// Workspace layouts: psi (incident waves) natural [y][x]; every k-space array private to these
+// Workspace layouts: psi (incident waves) in layout-R thread order as 16-byte pairs, [n1 / 2][tid] float4 =
+// (v[n1], v[n1 + 1]) -- written and read with one 16-byte access per two rows; every k-space array private to these
 // kernels (P^, Psi, the kept spectra, the seed weights, G^_P) in "thread order" [register][tid], which
 // is perfectly coalesced in layout K.  Same scaling conventions as pty_kernels.cuh (Ex carries 1/N,
 // Mx carries 1/N^2).
 #pragma once
+#ifndef PTY_BWD_SPLIT
+#define PTY_BWD_SPLIT 0
+#endif
 #include "pty_fft128.cuh"
 #include "pty_kernels.cuh"
 
@@ -29,22 +33,52 @@ PTY_DEV void block_accumulate128(const Cta128& c, int slot, float v) {
 // Fetch 32 float2 per thread (rows n1 = 0..31 at stride `stride` float2 from p) into the tensor-memory
 // staging block, four rows per tick: tick K (0..7) issues the loads of rows 4 K .. 4 K + 3, tick K + 1
 // parks them.  Nine ticks: everything is parked before the inverse transform's last exchange.
+// STREAM: the source is a saved wave in thread order (p = the thread's first float4, stride in float4 between pairs).
+// Two schedules: tick<K> puts all eight chunks into one inverse transform (the first slice of an item);
+// tick_fwd<K> / tick_inv<K> spread them over the forward transform that precedes the inverse (chunks 0-3, one
+// every three ticks) and the inverse itself (chunks 4-7, one every two ticks), which doubles the time between
+// a load and its park.  The staging block is free during the forward transform: its previous content was consumed
+// by the pointwise step just before.
 template <bool STREAM> struct Fetch32 {
     const float2* p;
     size_t stride;
     unsigned tm;
+    bool on;
     float2 buf[4];
-    template <int K> PTY_DEV void tick() {
-        if (K > 0 && K <= 8) tmem_st4(tm + 8 * (K - 1), buf);
-        if (K < 8) {
+    template <int C> PTY_DEV void issue() {
+        if (STREAM) {
+            const float4* p4 = reinterpret_cast<const float4*>(p);
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-                buf[i] = STREAM ? ld_stream2_pinned(p + (size_t)(4 * K + i) * stride) : ldg2_pinned(p + (size_t)(4 * K + i) * stride);
+            for (int i = 0; i < 2; ++i) {
+                const float4 t = ld_stream4_pinned(p4 + (size_t)(2 * C + i) * stride);
+                buf[2 * i] = make_float2(t.x, t.y);
+                buf[2 * i + 1] = make_float2(t.z, t.w);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) buf[i] = ldg2_pinned(p + (size_t)(4 * C + i) * stride);
         }
+    }
+    template <int C> PTY_DEV void park() { tmem_st4(tm + 8 * C, buf); }
+    template <int K> PTY_DEV void tick() {
+        if (K > 0 && K <= 8) park<(K > 0 && K <= 8) ? K - 1 : 0>();
+        if (K < 8) issue<K < 8 ? K : 0>();
+    }
+    template <int K> PTY_DEV void tick_fwd() {
+        if (!on) return;
+        if (K == 3 || K == 6 || K == 9 || K == 12) park<(K % 3 == 0 && K >= 3) ? K / 3 - 1 : 0>();
+        if (K == 0 || K == 3 || K == 6 || K == 9) issue<(K % 3 == 0 && K <= 9) ? K / 3 : 0>();
+    }
+    template <int K> PTY_DEV void tick_inv() {
+        if (K == 2 || K == 4 || K == 6 || K == 8) park<(K % 2 == 0 && K >= 2) ? 3 + K / 2 : 0>();
+        if (K == 0 || K == 2 || K == 4 || K == 6) issue<(K % 2 == 0 && K <= 6) ? 4 + K / 2 : 0>();
     }
     // rows 4 K .. 4 K + 3 (tmem_wait_st() once before the first take)
     template <int K> PTY_DEV void take(float2 (&o)[4]) { tmem_ld4(tm + 8 * K, o); tmem_wait_ld(); }
 };
+
+template <class F> struct FetchFwdHalf { F& f; template <int K> PTY_DEV void tick() { f.template tick_fwd<K>(); } };
+template <class F> struct FetchInvHalf { F& f; template <int K> PTY_DEV void tick() { f.template tick_inv<K>(); } };
 
 // Fetch 32 float2 per thread into the EXCHANGE block while it is free (after a FREE exchange), eight rows
 // per tick of the last fft32 of the inverse transform: ticks 0..3 issue rows 8 J .. 8 J + 7, ticks 1, 2, 3
@@ -80,6 +114,9 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     fo.p = A.object + ((size_t)ry + g) * A.W + rx + cc;
     fo.stride = (size_t)4 * A.W;
     fo.tm = c.tm_s();
+    fo.on = true;
+    FetchFwdHalf<Fetch32<false>> fo_fwd{fo};
+    FetchInvHalf<Fetch32<false>> fo_inv{fo};
     NoBg nobg;
     {   // a2: psi_0 = F^-1[E . P^]   (K -> R)
         const float2* Ph = A.probe_hat + (size_t)m * NN + c.tid;
@@ -90,23 +127,24 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
     }
     for (int s = 0; s < A.Nz; ++s) {
         {   // a3 + a4 (R): keep psi_{s-1}, phi_s = O_b[s] psi_{s-1}
-            float2* save = A.ws_psi + (bm * A.Nz + s) * NN + g * N + cc;
+            float4* save = reinterpret_cast<float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + c.tid;
             tmem_wait_st();
 #define PTY_OBJ_CHUNK(K)                                                   \
             {                                                              \
                 float2 o[4];                                               \
                 fo.template take<K>(o);                                    \
-                _Pragma("unroll") for (int i = 0; i < 4; ++i) {            \
-                    st_stream2(save + 4 * (4 * K + i) * N, v[4 * K + i]);  \
+                st_stream4(save + (2 * K) * F128::NT, v[4 * K], v[4 * K + 1]);          \
+                st_stream4(save + (2 * K + 1) * F128::NT, v[4 * K + 2], v[4 * K + 3]);  \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i)              \
                     v[4 * K + i] = cmul(v[4 * K + i], o[i]);               \
-                }                                                          \
             }
             PTY_OBJ_CHUNK(0) PTY_OBJ_CHUNK(1) PTY_OBJ_CHUNK(2) PTY_OBJ_CHUNK(3)
             PTY_OBJ_CHUNK(4) PTY_OBJ_CHUNK(5) PTY_OBJ_CHUNK(6) PTY_OBJ_CHUNK(7)
 #undef PTY_OBJ_CHUNK
             fo.p += (size_t)A.H * A.W;
         }
-        f128_forward(c, v);
+        fo.on = s < A.Nz - 1;
+        f128_forward<true>(c, v, fo_fwd);
         if (s == A.Nz - 1) break;
         {   // a4 (K): propagator M = My[ky] Mx[kx] (/N^2); keep the spectrum F[psi_s]
             float2* hat = A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + s) * NN + c.tid : nullptr;
@@ -117,7 +155,7 @@ PTY_DEV void fwd_body128(const KArgs& A, const Cta128& c, int item) {
                 if (hat) st_stream2(hat + r * F128::NT, v[r]);
             }
         }
-        f128_inverse<false>(c, v, fo, nobg);
+        f128_inverse<false>(c, v, fo_inv, nobg);
     }
     // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2 (transposed through X so that the reductions into the
     // natural [ky][kx] array are coalesced)
@@ -153,9 +191,12 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
     // transform that precedes their use: psi (HBM stream) over its 9 ticks into the staging block, the
     // object rows over the last fft32 into the exchange block once it is free.
     Fetch32<true> fp;
-    fp.p = A.ws_psi + (bm * A.Nz + (A.Nz - 1)) * NN + g * N + cc;
-    fp.stride = (size_t)4 * N;
+    fp.p = A.ws_psi + (bm * A.Nz + (A.Nz - 1)) * NN + 2 * c.tid;
+    fp.stride = F128::NT;
     fp.tm = c.tm_s();
+    fp.on = true;
+    FetchFwdHalf<Fetch32<true>> fp_fwd{fp};
+    FetchInvHalf<Fetch32<true>> fp_inv{fp};
     Fetch32x8 fo;
     fo.p = A.object + ((size_t)(A.Nz - 1) * A.H + ry + g) * A.W + rx + cc;
     fo.stride = (size_t)4 * A.W;
@@ -199,7 +240,12 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
             fp.p -= (size_t)N * N;
             fo.p -= (size_t)A.H * A.W;
         }
+#if PTY_BWD_SPLIT
+        fp.on = s > 0;
+        f128_forward<false>(c, v, fp_fwd);
+#else
         f128_forward<false>(c, v, nobg);
+#endif
         if (s == 0) break;
         {   // a9, a13 (K): D-sums against the kept spectrum, then conj(M)
             const float2 my = c.My[cc];
@@ -219,7 +265,11 @@ PTY_DEV void bwd_body128(const KArgs& A, const Cta128& c, int item) {
 #pragma unroll
             for (int r = 0; r < 32; ++r) v[r] = cmulc(cmul(my, c.Mx[c.kx(r)]), v[r]);
         }
+#if PTY_BWD_SPLIT
+        f128_inverse<true>(c, v, fp_inv, fo);
+#else
         f128_inverse<true>(c, v, fp, fo);
+#endif
     }
     // a11, a12 (K): g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
     const float2* Ph = A.probe_hat + (size_t)m * NN + c.tid;

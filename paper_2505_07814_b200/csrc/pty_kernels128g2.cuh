@@ -1,0 +1,460 @@
+// pty_kernels128g2.cuh -- N = 128 forward and adjoint bodies, TWO independent items per CTA.
+//
+// A CTA of 512 threads is two groups of 256 threads (8 warps, two per SM sub-partition); each group owns
+// one (position, mode) item.  The group's 128 x 128 wave lives in tensor memory (256 of the 512 TMEM columns)
+// and passes through the registers half at a time: a thread plays two of the four "roles" o = 2 gg + h of the
+// 512-thread kernel (pty_fft128.cuh: role = the old thread-group index g), one after the other, 32 complex
+// values each.  All layouts (R, K, thread-order workspace arrays) are those of pty_kernels128.cuh with g -> o.
+//
+//   TMEM, per group: four role blocks of 64 columns; block(q) holds the 32 values role q consumes next.
+//     forward exchange : role o writes its fft32 output into block(o) (chunk j = values 8 j .. 8 j + 7 is for
+//                        role j); role o' reads chunk o' of every block.
+//     inverse exchange : role o' writes the chunk for role q into block(q)[chunk o'] -- exactly the slots it
+//                        has just read in the forward direction (a 4 x 4 in-place chunk transpose), so the
+//                        k-space pointwise step between a forward and an inverse transform needs no extra space.
+//   The two threads of a lane that share a role block are the same lane of warps w and w + 4 of the group:
+//   same SM sub-partition, same TMEM lane; their barrier has 64 threads.
+//   Shared memory: ONE transpose buffer X (128 x 129 float2) for the CTA, handed back and forth between the
+//   groups with named barriers (acquire = bar.sync, release = bar.arrive, 512 = 256 + 256 threads).  Each group
+//   holds X for about a third of its time, so the groups settle half a period apart: while one streams its
+//   loads, stores and reductions (LSU and latency bound), the other runs butterflies (FP32 pipe bound).
+#pragma once
+#include "pty_fft128.cuh"
+#include "pty_kernels.cuh"
+
+namespace pty {
+
+struct G2Smem {
+    static constexpr size_t xch_bytes = F128::xch_bytes;
+    // twg[128] | per group: Ey, Ex, My, Mx [128 each] float2, red[64] float | TMEM base
+    static constexpr size_t group_bytes = 4 * 128 * sizeof(float2) + 64 * sizeof(float);
+    static constexpr size_t bytes = xch_bytes + 128 * sizeof(float2) + 2 * group_bytes + 16;
+};
+
+struct G2 {
+    int tid, t, G, gg, c, smsp;
+    float2* X;
+    float2* twg;
+    float2 *Ey, *Ex, *My, *Mx;
+    float* red;
+    unsigned tl;     // TMEM address: this thread's lane quarter, first column of the group (256 G)
+    PTY_DEV unsigned blk(int q) const { return tl + 64u * (unsigned)q; }
+    PTY_DEV int kx(int o, int r) const { return 8 * o + (r & 7) + 32 * (r >> 3); }
+    PTY_DEV void pair_sync() const {
+        tmem_fence_before_sync();
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + 4 * G + smsp) : "memory");
+        tmem_fence_after_sync();
+    }
+    PTY_DEV void grp_sync() const { asm volatile("bar.sync %0, 256;" ::"r"(9 + G) : "memory"); }
+    PTY_DEV void acquireX() const { asm volatile("bar.sync %0, 512;" ::"r"(11 + G) : "memory"); }
+    PTY_DEV void releaseX() const { asm volatile("bar.arrive %0, 512;" ::"r"(11 + (G ^ 1)) : "memory"); }
+};
+
+PTY_DEV G2 make_g2(unsigned char* smem) {
+    G2 c;
+    c.tid = threadIdx.x; c.t = c.tid & 255; c.G = c.tid >> 8; c.gg = (c.tid >> 7) & 1; c.c = c.tid & 127;
+    c.smsp = (c.tid >> 5) & 3;
+    c.X = reinterpret_cast<float2*>(smem);
+    float2* tab = reinterpret_cast<float2*>(smem + G2Smem::xch_bytes);
+    c.twg = tab;
+    unsigned char* gp = reinterpret_cast<unsigned char*>(tab + 128) + (size_t)c.G * G2Smem::group_bytes;
+    float2* gt = reinterpret_cast<float2*>(gp);
+    c.Ey = gt; c.Ex = gt + 128; c.My = gt + 256; c.Mx = gt + 384;
+    c.red = reinterpret_cast<float*>(gt + 512);
+    unsigned* tbase = reinterpret_cast<unsigned*>(reinterpret_cast<unsigned char*>(tab + 128) + 2 * G2Smem::group_bytes);
+    if ((threadIdx.x >> 5) == 0) tmem_alloc512(tbase);
+    for (int j = c.tid; j < 128; j += 512) {
+        float s, co;
+        const int gi = j >> 2, qq = j & 3;
+        sincospi_f(2.0f * (float)(qq * gi) / 128.0f, &s, &co);
+        c.twg[j] = make_float2(co, -s);
+    }
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    c.tl = *tbase + ((32u * (unsigned)c.smsp) << 16) + 256u * (unsigned)c.G;
+    return c;
+}
+
+PTY_DEV void release_g2(unsigned char* smem) {
+    tmem_fence_before_sync();
+    __syncthreads();
+    float2* tab = reinterpret_cast<float2*>(smem + G2Smem::xch_bytes);
+    unsigned* tbase = reinterpret_cast<unsigned*>(reinterpret_cast<unsigned char*>(tab + 128) + 2 * G2Smem::group_bytes);
+    if ((threadIdx.x >> 5) == 0) tmem_dealloc512(*tbase);
+}
+
+// ------------------------------------------------------------------------------ radix-4 stage with twiddles
+// DIR < 0: v[8 q + i] -> twiddle W128^(q (8 o + i)) -> radix-4 over q -> v[8 k2 + i]   (forward)
+// DIR > 0: v[8 k2 + i] -> inverse radix-4 over k2 -> conj twiddle -> v[8 q + i]         (inverse)
+template <int DIR> PTY_DEV void g2_radix4(const G2& c, int o, float2 (&v)[32]) {
+    const float4* tw = reinterpret_cast<const float4*>(c.twg + 32 * o);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float4 t01 = tw[2 * i], t23 = tw[2 * i + 1];
+        if (DIR < 0) {
+            float2 a0 = v[i];
+            float2 a1 = cmul(v[8 + i], make_float2(t01.z, t01.w));
+            float2 a2 = cmul(v[16 + i], make_float2(t23.x, t23.y));
+            float2 a3 = cmul(v[24 + i], make_float2(t23.z, t23.w));
+            bfly4<-1>(a0, a1, a2, a3);
+            v[i] = a0; v[8 + i] = a1; v[16 + i] = a2; v[24 + i] = a3;
+        } else {
+            float2 a0 = v[i], a1 = v[8 + i], a2 = v[16 + i], a3 = v[24 + i];
+            bfly4<+1>(a0, a1, a2, a3);
+            v[i] = a0;
+            v[8 + i] = cmulc(make_float2(t01.z, t01.w), a1);
+            v[16 + i] = cmulc(make_float2(t23.x, t23.y), a2);
+            v[24 + i] = cmulc(make_float2(t23.z, t23.w), a3);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------ TMEM role blocks
+PTY_DEV void g2_ld_own(const G2& c, int o, float2 (&v)[32]) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) tmem_ld8(c.blk(o) + 16 * j, v, 8 * j);
+    tmem_wait_ld();
+}
+PTY_DEV void g2_st_own(const G2& c, int o, float2 (&v)[32]) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) tmem_st8(c.blk(o) + 16 * j, v, 8 * j);
+}
+PTY_DEV void g2_ld_slots(const G2& c, int o, float2 (&v)[32]) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) tmem_ld8(c.blk(q) + 16 * o, v, 8 * q);
+    tmem_wait_ld();
+}
+PTY_DEV void g2_st_slots(const G2& c, int o, float2 (&v)[32]) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) tmem_st8(c.blk(q) + 16 * o, v, 8 * q);
+}
+
+// ------------------------------------------------------------------------------ transform phases
+// Inverse transform up to the last exchange: role blocks (k space, after the inverse x radix-4) ->
+// x fft32^-1 -> X -> y radix-4^-1 -> role blocks.  The caller then runs, per role, g2_ld_own + fft32<+1>.
+// FIRST: this is the CTA's very first use of X by group 0 (nothing to acquire).
+PTY_DEV void g2_inverse_head(const G2& c, float2 (&v)[32], bool first) {
+    constexpr int P = F128::P;
+    NoBg bg;
+    c.pair_sync();
+    if (!first) c.acquireX();
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+        const int o = 2 * c.gg + h;
+        g2_ld_own(c, o, v);
+        fft32<+1, 0>(v, bg);
+        float2* s = c.X + c.c * P + o;
+#pragma unroll
+        for (int n = 0; n < 32; ++n) s[4 * n] = v[n];
+    }
+    c.grp_sync();
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+        const int o = 2 * c.gg + h;
+        const float2* s = c.X + (8 * o) * P + c.c;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            v[i] = s[i * P];
+            v[8 + i] = s[(i + 32) * P];
+            v[16 + i] = s[(i + 64) * P];
+            v[24 + i] = s[(i + 96) * P];
+        }
+        if (h == 1) c.releaseX();
+        g2_radix4<+1>(c, o, v);
+        g2_st_slots(c, o, v);
+    }
+    tmem_wait_st();
+    c.pair_sync();
+}
+
+// Forward transform after the per-role fft32<-1> + g2_st_own of the caller: role blocks -> y radix-4 -> X ->
+// x fft32 -> role blocks.  The caller then runs, per role, g2_ld_slots + g2_radix4<-1> (k space, layout K).
+PTY_DEV void g2_forward_tail(const G2& c, float2 (&v)[32]) {
+    constexpr int P = F128::P;
+    NoBg bg;
+    tmem_wait_st();
+    c.pair_sync();
+    c.acquireX();
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+        const int o = 2 * c.gg + h;
+        g2_ld_slots(c, o, v);
+        g2_radix4<-1>(c, o, v);
+        float2* s = c.X + (8 * o) * P + c.c;
+#pragma unroll
+        for (int r = 0; r < 32; ++r) s[((r & 7) + 32 * (r >> 3)) * P] = v[r];
+    }
+    c.grp_sync();
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+        const int o = 2 * c.gg + h;
+        const float2* s = c.X + c.c * P + o;
+#pragma unroll
+        for (int n2 = 0; n2 < 8; ++n2) {
+            v[n2] = s[4 * n2];
+            v[8 + n2] = s[4 * (8 + n2)];
+            v[16 + n2] = s[4 * (16 + n2)];
+            v[24 + n2] = s[4 * (24 + n2)];
+        }
+        if (h == 1) c.releaseX();
+        fft32<-1, 0>(v, bg);
+        g2_st_own(c, o, v);
+    }
+    tmem_wait_st();
+    c.pair_sync();
+}
+
+PTY_DEV void g2_accumulate(const G2& c, int slot, float v) {
+    v = warp_sum(v);
+    if (warp_leader()) red_add_shared(c.red + slot, v);
+}
+
+// ------------------------------------------------------------------------------ forward (a2-a5)
+// item = b M + m; live = false for the padding item of an odd grid (same control flow, no global writes).
+PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
+    constexpr int N = 128, NT = F128::NT, P = F128::P;
+    const int b = item / A.M, m = item % A.M;
+    int ry, rx;
+    setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
+    c.grp_sync();
+    const size_t NN = (size_t)N * N;
+    const size_t bm = (size_t)b * A.M + m;
+    float2 v[32];
+    NoBg bg;
+    {   // a2 (K): E . P^ -> inverse x radix-4 -> role blocks
+        const float2 ey = c.Ey[c.c];
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            const float2* Ph = A.probe_hat + (size_t)m * NN + 128 * o + c.c;
+#pragma unroll
+            for (int r = 0; r < 32; ++r) v[r] = cmul(cmul(ldg2(Ph + r * NT), ey), c.Ex[c.kx(o, r)]);
+            g2_radix4<+1>(c, o, v);
+            g2_st_slots(c, o, v);
+        }
+        tmem_wait_st();
+    }
+    bool first = (c.G == 0);
+    for (int s = 0; s < A.Nz; ++s) {
+        g2_inverse_head(c, v, first);
+        first = false;
+        // a3 + a4 (R): psi_{s-1} = fft32^-1, keep it, phi_s = O_b[s] psi_{s-1}, first stage of the forward y transform
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            const float2* obj = A.object + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
+            const size_t ostride = (size_t)4 * A.W;
+            float2 oa[8], ob[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) oa[i] = ldg2_pinned(obj + (size_t)i * ostride);
+            g2_ld_own(c, o, v);
+            fft32<+1, 0>(v, bg);
+            float4* save = reinterpret_cast<float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 128 * o + c.c;
+#define PTY_G2_CHUNK(J, CUR, NXT)                                                                       \
+            {                                                                                           \
+                if (J < 3) { _Pragma("unroll") for (int i = 0; i < 8; ++i)                              \
+                    NXT[i] = ldg2_pinned(obj + (size_t)(8 * (J + 1) + i) * ostride); }                  \
+                _Pragma("unroll") for (int i = 0; i < 8; i += 2)                                        \
+                    if (live) st_stream4(save + (4 * J + i / 2) * NT, v[8 * J + i], v[8 * J + i + 1]);  \
+                _Pragma("unroll") for (int i = 0; i < 8; ++i) v[8 * J + i] = cmul(v[8 * J + i], CUR[i]); \
+            }
+            PTY_G2_CHUNK(0, oa, ob) PTY_G2_CHUNK(1, ob, oa) PTY_G2_CHUNK(2, oa, ob) PTY_G2_CHUNK(3, ob, oa)
+#undef PTY_G2_CHUNK
+            fft32<-1, 0>(v, bg);
+            g2_st_own(c, o, v);
+        }
+        g2_forward_tail(c, v);
+        if (s == A.Nz - 1) break;
+        // a4 (K): propagator, inverse x radix-4, in-place slots
+        const float2 my = c.My[c.c];
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            g2_ld_slots(c, o, v);
+            g2_radix4<-1>(c, o, v);
+            float2* hat = A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + s) * NN + 128 * o + c.c : nullptr;
+#pragma unroll
+            for (int r = 0; r < 32; ++r) {
+                v[r] = cmul(v[r], cmul(my, c.Mx[c.kx(o, r)]));
+                if (hat && live) st_stream2(hat + r * NT, v[r]);
+            }
+            g2_radix4<+1>(c, o, v);
+            g2_st_slots(c, o, v);
+        }
+        tmem_wait_st();
+    }
+    // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2 (through X so that the reductions into [ky][kx] are coalesced)
+    float* Xf = reinterpret_cast<float*>(c.X);
+    c.acquireX();
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+        const int o = 2 * c.gg + h;
+        g2_ld_slots(c, o, v);
+        g2_radix4<-1>(c, o, v);
+        float2* Psi = A.ws_Psi + bm * NN + 128 * o + c.c;
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {
+            const float2 p = cscale(v[r], 1.0f / N);
+            if (live) st_stream2(Psi + r * NT, p);
+            Xf[c.c * P + c.kx(o, r)] = p.x * p.x + p.y * p.y;
+        }
+    }
+    c.grp_sync();
+    float* Ib = A.I + (size_t)b * NN;
+    if (live) {
+#pragma unroll 8
+        for (int j = 0; j < 64; ++j) {
+            const int idx = j * 256 + c.t;
+            red_add(Ib + idx, Xf[(idx >> 7) * P + (idx & 127)]);
+        }
+    }
+    c.releaseX();
+    if (c.G == 0) c.acquireX();      // consume group 1's last release
+}
+
+// ------------------------------------------------------------------------------ adjoint (a7-a13)
+PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
+    constexpr int N = 128, NT = F128::NT;
+    const int b = item / A.M, m = item % A.M;
+    int ry, rx;
+    setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
+    c.grp_sync();
+    const size_t NN = (size_t)N * N;
+    const size_t bm = (size_t)b * A.M + m;
+    float2 v[32];
+    NoBg bg;
+    {   // a7, a8 (K): g_Psi = w Psi, inverse x radix-4 -> role blocks
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            const float2* Psi = A.ws_Psi + bm * NN + 128 * o + c.c;
+            const float* Wt = A.seed_w + (size_t)b * NN + 128 * o + c.c;
+#pragma unroll
+            for (int r = 0; r < 32; ++r) v[r] = cscale(ld_stream2(Psi + r * NT), ldg1(Wt + r * NT));
+            g2_radix4<+1>(c, o, v);
+            g2_st_slots(c, o, v);
+        }
+        tmem_wait_st();
+    }
+    float acc_ky = 0.f, acc_kx = 0.f, acc_k2 = 0.f;
+    bool first = (c.G == 0);
+    for (int s = A.Nz - 1; s >= 0; --s) {
+        g2_inverse_head(c, v, first);
+        first = false;
+        // a9, a10 (R): g = fft32^-1; g_object patch += conj(psi_{s-1}) g; g <- conj(O_b[s]) g; forward y first stage
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            const float2* obj = A.object + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
+            float2* gobj = A.g_object + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
+            const size_t ostride = (size_t)4 * A.W;
+            const float4* psi = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 128 * o + c.c;
+            float2 oa[4], ob[4];
+            float4 pa[2], pb[2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) pa[i] = ld_stream4_pinned(psi + (size_t)i * NT);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) oa[i] = ldg2_pinned(obj + (size_t)i * ostride);
+            g2_ld_own(c, o, v);
+            fft32<+1, 0>(v, bg);
+#define PTY_G2_BCHUNK(J, OC, ON, PC, PN)                                                                  \
+            {                                                                                             \
+                if (J < 7) {                                                                              \
+                    _Pragma("unroll") for (int i = 0; i < 2; ++i)                                         \
+                        PN[i] = ld_stream4_pinned(psi + (size_t)(2 * (J + 1) + i) * NT);                  \
+                    _Pragma("unroll") for (int i = 0; i < 4; ++i)                                         \
+                        ON[i] = ldg2_pinned(obj + (size_t)(4 * (J + 1) + i) * ostride);                   \
+                }                                                                                         \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i) {                                           \
+                    const float4 pp = PC[i >> 1];                                                         \
+                    const float2 ps = (i & 1) ? make_float2(pp.z, pp.w) : make_float2(pp.x, pp.y);        \
+                    if (live) red_add2(gobj + (size_t)(4 * J + i) * ostride, cmulc(ps, v[4 * J + i]));    \
+                    v[4 * J + i] = cmulc(OC[i], v[4 * J + i]);                                            \
+                }                                                                                         \
+            }
+            PTY_G2_BCHUNK(0, oa, ob, pa, pb) PTY_G2_BCHUNK(1, ob, oa, pb, pa) PTY_G2_BCHUNK(2, oa, ob, pa, pb)
+            PTY_G2_BCHUNK(3, ob, oa, pb, pa) PTY_G2_BCHUNK(4, oa, ob, pa, pb) PTY_G2_BCHUNK(5, ob, oa, pb, pa)
+            PTY_G2_BCHUNK(6, oa, ob, pa, pb) PTY_G2_BCHUNK(7, ob, oa, pb, pa)
+#undef PTY_G2_BCHUNK
+            fft32<-1, 0>(v, bg);
+            g2_st_own(c, o, v);
+        }
+        g2_forward_tail(c, v);
+        if (s == 0) break;
+        // a9, a13 (K): D-sums against the kept spectrum, conj(M), inverse x radix-4, in-place slots
+        const float2 my = c.My[c.c];
+        const float kyf = kp_of<N>(c.c);
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            g2_ld_slots(c, o, v);
+            g2_radix4<-1>(c, o, v);
+            if (A.save_hat) {
+                const float2* hat = A.ws_hat + (bm * (A.Nz - 1) + (s - 1)) * NN + 128 * o + c.c;
+#pragma unroll
+                for (int r = 0; r < 32; ++r) {
+                    const float2 hs = ld_stream2(hat + r * NT);
+                    const float d = hs.x * v[r].y - hs.y * v[r].x;          // Im(conj(psi^) g^)
+                    const float kxf = kp_of<N>(c.kx(o, r));
+                    acc_ky += d * kyf;
+                    acc_kx += d * kxf;
+                    acc_k2 += d * (kyf * kyf + kxf * kxf);
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < 32; ++r) v[r] = cmulc(cmul(my, c.Mx[c.kx(o, r)]), v[r]);
+            g2_radix4<+1>(c, o, v);
+            g2_st_slots(c, o, v);
+        }
+        tmem_wait_st();
+    }
+    // a11, a12 (K): g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
+    float accy = 0.f, accx = 0.f;
+    {
+        const float2 ey = c.Ey[c.c];
+        const float kyf = kp_of<N>(c.c);
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            g2_ld_slots(c, o, v);
+            g2_radix4<-1>(c, o, v);
+            const float2* Ph = A.probe_hat + (size_t)m * NN + 128 * o + c.c;
+            float2* GP = A.GP_hat + (size_t)m * NN + 128 * o + c.c;
+#pragma unroll
+            for (int r = 0; r < 32; ++r) {
+                const int kx = c.kx(o, r);
+                const float2 gg = v[r];
+                const float2 e = cmul(ey, c.Ex[kx]);                     // E / N
+                if (live) red_add2(GP + r * NT, cmulc(e, gg));
+                const float2 ep = cmul(e, ldg2(Ph + r * NT));
+                const float t = gg.x * ep.y - gg.y * ep.x;               // Im(conj(g^_0) E P^)
+                accy += kyf * t;
+                accx += kp_of<N>(kx) * t;
+            }
+        }
+    }
+    g2_accumulate(c, 0, accy);
+    g2_accumulate(c, 1, accx);
+    if (A.save_hat) {
+        g2_accumulate(c, 2, acc_ky);
+        g2_accumulate(c, 3, acc_kx);
+        g2_accumulate(c, 4, acc_k2);
+    }
+    c.grp_sync();
+    if (c.t == 0 && live) {
+        const float two_pi = 6.283185307179586f;
+        if (A.g_pos) {
+            red_add(A.g_pos + 2 * b, two_pi * c.red[0]);
+            red_add(A.g_pos + 2 * b + 1, two_pi * c.red[1]);
+        }
+        if (A.save_hat) {
+            red_add(A.dsum + 4 * b, c.red[2]);
+            red_add(A.dsum + 4 * b + 1, c.red[3]);
+            red_add(A.dsum + 4 * b + 2, c.red[4]);
+        }
+    }
+    if (c.G == 0) c.acquireX();      // consume group 1's last release
+}
+
+}  // namespace pty

@@ -11,6 +11,7 @@
 #include "../../include/pty.h"
 #include "pty_kernels.cuh"
 #include "pty_kernels128.cuh"
+#include "pty_kernels128g2.cuh"
 
 namespace cg = cooperative_groups;
 using namespace pty;
@@ -90,6 +91,22 @@ __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128_kernel(const KArgs A) 
     extern __shared__ __align__(16) unsigned char smem[];
     bwd_body128(A, make_cta128(smem), blockIdx.x);
     release_cta128(smem);
+}
+
+// N = 128, two items per CTA (pty_kernels128g2.cuh): group G of CTA x owns item 2 x + G
+__global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const G2 c = make_g2(smem);
+    const int n = A.B * A.M, item = 2 * blockIdx.x + c.G;
+    fwd_body_g2(A, c, min(item, n - 1), item < n);
+    release_g2(smem);
+}
+__global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_kernel(const KArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const G2 c = make_g2(smem);
+    const int n = A.B * A.M, item = 2 * blockIdx.x + c.G;
+    bwd_body_g2(A, c, min(item, n - 1), item < n);
+    release_g2(smem);
 }
 
 // a0: P^ = F[P] / N in thread order; a11: g_probe = F^-1[G^_P] / N (one CTA per mode)
@@ -334,6 +351,7 @@ struct pty_plan {
     const void *f_object, *f_probe, *f_positions, *f_tilt, *f_meas;
     int32_t f_B;
 
+    bool g2;                     // N = 128: two items per CTA (pty_kernels128g2.cuh)
     bool reg128;                 // N = 128 on the register-resident FFT (default) or the shared-memory passes
     // optional kernel timing (pty_profile)
     bool profiling;
@@ -422,12 +440,16 @@ struct ScopedTimer {
 
 template <class SH> cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 0, st);
+    if (SH::N == 128 && p->reg128 && p->g2)
+        return launch(p, pty_fwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
     if (SH::N == 128 && p->reg128)
         return launch(p, pty_fwd128_kernel, A.B * A.M, F128::NT, F128::smem_bytes, 1, st, A);
     return launch(p, pty_fwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
 template <class SH> cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 1, st);
+    if (SH::N == 128 && p->reg128 && p->g2)
+        return launch(p, pty_bwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
     if (SH::N == 128 && p->reg128)
         return launch(p, pty_bwd128_kernel, A.B * A.M, F128::NT, F128::smem_bytes, 1, st, A);
     return launch(p, pty_bwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
@@ -599,6 +621,12 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
     if (e == cudaSuccess) e = PTY_DISPATCH_N(p, set_smem_attrs<Shape<64>>(), set_smem_attrs<Shape<128>>(), set_smem_attrs<Shape<256>>());
     const char* sel = getenv("PTY_FFT128");          // "smem" selects the shared-memory-pass kernels for N = 128
     p->reg128 = !(sel && strcmp(sel, "smem") == 0);
+    p->g2 = sel && strcmp(sel, "g2") == 0;
+    if (e == cudaSuccess && dims->N == 128) {
+        e = cudaFuncSetAttribute(pty_fwd128g2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_bwd128g2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+    }
     if (e == cudaSuccess && dims->N == 128) {
         e = cudaFuncSetAttribute(pty_fwd128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
         if (e == cudaSuccess)

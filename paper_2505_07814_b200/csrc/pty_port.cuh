@@ -97,6 +97,14 @@ PTY_DEV float2 ld_stream2_pinned(const float2* p) {
     return v;
 }
 
+// 16-byte streaming accesses (two complex values): the saved waves of the N = 128 register path
+PTY_DEV float4 ld_stream4_pinned(const float4* p) {
+    float4 v;
+    asm volatile("ld.global.cs.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+PTY_DEV void st_stream4(float4* p, float2 a, float2 b) { __stcs(p, make_float4(a.x, a.y, b.x, b.y)); }
+
 PTY_DEV void sincospi_f(float x, float* s, float* c) { sincospif(x, s, c); }
 PTY_DEV float rsqrt_f(float x) { return rsqrtf(x); }
 }  // namespace pty
