@@ -315,12 +315,18 @@ def main():
             kern[name] = {"avg_ms": ms / n, "launches": n, "tflops": flops_launch / (ms / n * 1e-3) / 1e12}
     dom = max(kern, key=lambda k: kern[k]["avg_ms"]) if kern else None
     roofline = None
+    fma_scalar = binding.fma_peak(local, packed=False)     # measured FP32 FMA rate on this GPU, after the timed region
+    fma_packed = binding.fma_peak(local, packed=True)
     if dom:
         a = kern[dom]["tflops"]
-        roofline = {"bound": "alu", "kernel": f"pty_{dom}_kernel<Shape<{cfg.N}>>", "achieved": a, "peak": peak_tf,
+        roofline = {"bound": "alu", "kernel": (f"pty_{dom}128g2_kernel" if cfg.N == 128 and os.environ.get("PTY_FFT128") in (None, "", "g2")
+                               else f"pty_{dom}_kernel<Shape<{cfg.N}>>"), "achieved": a, "peak": peak_tf,
                     "unit": "TFLOP/s", "frac": a / peak_tf, "traffic": None,
                     "peak_source": f"{n_sms} SMs x 128 FP32 lanes x 2 flop x clocks.max.sm {sm_max:.0f} MHz "
                                    "(nominal FP32 FMA peak; HBM is not the bound, DESIGN.md)",
+                    "peak_measured_fma": {"scalar_ffma_tflops": fma_scalar, "packed_ffma2_tflops": fma_packed,
+                                          "frac_of_measured": a / max(fma_scalar, fma_packed),
+                                          "how": "pty_fma_peak: independent FFMA / FFMA2 chains on every SM"},
                     "algorithmic_flops_per_launch": flops_launch, "avg_launch_ms": kern[dom]["avg_ms"],
                     "kernels": kern,
                     "whole_step_frac_of_fft_roofline": value * fft_flops_per_pattern(cfg, 0) / world / 1e12 / peak_tf,
@@ -344,9 +350,9 @@ def main():
         import oracle
         cores = len(os.sched_getaffinity(0))
         geom = oracle.Geometry(cfg.dz, cfg.lam, cfg.dx)
-        per_pattern_s = {1: 0.002, 2: 0.03, 3: 0.07, 4: 0.14, 5: 1.4}[cfg.c]
-        n = int(max(4, min(B, round(20.0 * cores / per_pattern_s / cores / 8) * 1)))   # ~ 20 s of CPU work / 8
-        n = max(4, min(B, max(cores, n)))
+        # ~ 15 s of wall time: measured 0.22 s per pattern per worker on config 4 (16 workers: 4.6 patterns/s)
+        per_pattern_s = {1: 0.003, 2: 0.05, 3: 0.11, 4: 0.22, 5: 2.2}[cfg.c]
+        n = int(max(cores, min(B, round(15.0 * cores / per_pattern_s))))
         idx = synth.minibatch(cfg, 0, B)[:n]
         tilt_tr = tr["tilt"] if cfg.tilt_mode else None
         tilt_ev = ev["tilt"] if cfg.tilt_mode else None

@@ -167,6 +167,13 @@ int64_t pty_launch_count(const pty_plan* plan);
 const char* pty_last_error(const pty_plan* plan);
 
 /* Library version string, e.g. "pty-b200 0.1 (sm_100a)". */
+/* FP32 pipe microbenchmark ("measure an FMA microbenchmark peak and the clock actually held"):
+ * runs a kernel of independent scalar FFMA chains (packed = 0) or packed FFMA2 chains (packed = 1) on every SM of
+ * `device` for about 20 ms and writes the achieved TFLOP/s (2 flops per FMA lane-operation) to *tflops (host).
+ * Allocates and frees 4 bytes of device memory; synchronises the device.  Not part of the hot path: bench.py
+ * reports it beside the nominal peak.  Returns PTY_OK or PTY_ERR_CUDA / PTY_ERR_INVALID_ARG. */
+int pty_fma_peak(int32_t device, int32_t packed, double* tflops);
+
 const char* pty_version(void);
 
 #ifdef __cplusplus

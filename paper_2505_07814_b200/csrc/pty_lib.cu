@@ -585,7 +585,51 @@ int adam_launch(pty_plan* p, float* theta, const float* g, float* m, float* v, s
 }  // namespace
 
 // ============================================================================ C ABI
+// FP32 pipe microbenchmark: 16 independent chains per thread, 1024 iterations, 8 CTAs of 512 threads per SM
+template <int PACKED> __global__ void __launch_bounds__(512) pty_fma_peak_kernel(float* out, float a, float b, int iters) {
+    float2 x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = make_float2(threadIdx.x * 1e-3f + i, i * 0.5f);
+    const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (PACKED) x[i] = __ffma2_rn(x[i], a2, b2);
+            else { x[i].x = fmaf(x[i].x, a, b); x[i].y = fmaf(x[i].y, a, b); }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i].x + x[i].y;
+    if (s == 12345.678f) out[0] = s;
+}
+
 extern "C" {
+
+int pty_fma_peak(int32_t device, int32_t packed, double* tflops) {
+    if (!tflops) return PTY_ERR_INVALID_ARG;
+    cudaDeviceProp prop;
+    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) return PTY_ERR_CUDA;
+    float* d = nullptr;
+    if (cudaMalloc(&d, 4) != cudaSuccess) return PTY_ERR_CUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int grid = prop.multiProcessorCount * 8, iters = 1 << 16;
+    float best = 1e30f;
+    for (int r = 0; r < 3; ++r) {
+        cudaEventRecord(e0);
+        if (packed) pty_fma_peak_kernel<1><<<grid, 512>>>(d, 1.0001f, 0.5f, iters);
+        else pty_fma_peak_kernel<0><<<grid, 512>>>(d, 1.0001f, 0.5f, iters);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return PTY_ERR_CUDA; }
+        float ms; cudaEventElapsedTime(&ms, e0, e1);
+        if (r && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    *tflops = 2.0 * 16.0 * (double)iters * 512.0 * grid / (best * 1e-3) / 1e12;
+    return PTY_OK;
+}
 
 const char* pty_version(void) { return "pty-b200 0.1 (sm_100a)"; }
 
@@ -619,9 +663,11 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
         return fail(nullptr, PTY_ERR_UNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor);
     }
     if (e == cudaSuccess) e = PTY_DISPATCH_N(p, set_smem_attrs<Shape<64>>(), set_smem_attrs<Shape<128>>(), set_smem_attrs<Shape<256>>());
-    const char* sel = getenv("PTY_FFT128");          // "smem" selects the shared-memory-pass kernels for N = 128
+    // N = 128 kernel family: default = two items per CTA (pty_kernels128g2.cuh); PTY_FFT128=reg selects the
+    // one-item register-resident kernels (pty_kernels128.cuh), PTY_FFT128=smem the shared-memory-pass kernels
+    const char* sel = getenv("PTY_FFT128");
     p->reg128 = !(sel && strcmp(sel, "smem") == 0);
-    p->g2 = sel && strcmp(sel, "g2") == 0;
+    p->g2 = p->reg128 && !(sel && strcmp(sel, "reg") == 0);
     if (e == cudaSuccess && dims->N == 128) {
         e = cudaFuncSetAttribute(pty_fwd128g2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)

@@ -123,6 +123,20 @@ def test_parity_all_configs(pty, c, which, B):
           " ".join(f"{k} {v:.2e}" for k, v in errs.items()))
 
 
+@pytest.mark.parametrize("family", ["g2", "reg", "smem"])
+def test_n128_kernel_families(pty, family, monkeypatch):
+    """The three N = 128 kernel families (PTY_FFT128, read by pty_create): two items per CTA (default), one item
+    per CTA on the register FFT, shared-memory passes.  B x M is odd here (7 x 3 after trimming the probe), so
+    the two-item kernels run their padding item; with the dz gradient so that the kept spectra are covered."""
+    monkeypatch.setenv("PTY_FFT128", family)
+    cfg = synth.get_config(3, M=3)
+    case = make_case(3, "A", synth.minibatch(cfg, 2, cfg.B)[:7])
+    case = dict(case, cfg=cfg, probe=np.ascontiguousarray(case["probe"][:3]))
+    ref = oracle_grad(case)
+    res = run_gpu(pty, case, want_dz=True)
+    check_against_oracle(res, ref, case)
+
+
 def test_per_position_tilt_and_dz(pty):
     """tilt_mode 2 (one tilt per position) on the multislice config, with the dz gradient."""
     cfg = synth.get_config(3)
