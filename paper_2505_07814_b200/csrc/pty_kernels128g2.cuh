@@ -342,41 +342,64 @@ PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
     for (int s = A.Nz - 1; s >= 0; --s) {
         g2_inverse_head(c, v, first);
         first = false;
-        // a9, a10 (R): g = fft32^-1; g_object patch += conj(psi_{s-1}) g; g <- conj(O_b[s]) g; forward y first stage
+        // a9, a10 (R): g = fft32^-1; g_object patch += conj(psi_{s-1}) g; g <- conj(O_b[s]) g; forward y first stage.
+        // Park-then-stream: both roles' g goes back to its TMEM block first, which frees the 64 wave registers;
+        // the pointwise step then streams over the 16 chunks of 4 rows (two roles x 8) with the saved wave
+        // (HBM stream) and the object rows five chunks ahead in registers and g one chunk ahead from TMEM.
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
             const int o = 2 * c.gg + h;
-            const float2* obj = A.object + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
-            float2* gobj = A.g_object + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
-            const size_t ostride = (size_t)4 * A.W;
-            const float4* psi = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 128 * o + c.c;
-            float2 oa[4], ob[4];
-            float4 pa[2], pb[2];
-#pragma unroll
-            for (int i = 0; i < 2; ++i) pa[i] = ld_stream4_pinned(psi + (size_t)i * NT);
-#pragma unroll
-            for (int i = 0; i < 4; ++i) oa[i] = ldg2_pinned(obj + (size_t)i * ostride);
             g2_ld_own(c, o, v);
             fft32<+1, 0>(v, bg);
-#define PTY_G2_BCHUNK(J, OC, ON, PC, PN)                                                                  \
+            g2_st_own(c, o, v);
+        }
+        tmem_wait_st();
+        {
+            constexpr int D = 5;
+            const size_t ostride = (size_t)4 * A.W;
+            const float2* obj0 = A.object + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
+            float2* gobj0 = A.g_object + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
+            const float4* psi0 = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 256 * c.gg + c.c;
+            const unsigned tb0 = c.blk(2 * c.gg);
+            float4 pb[D][2];
+            float2 ob[D][4];
+            float2 gb[2][4];
+#define PTY_G2_ISSUE(J)                                                                                   \
             {                                                                                             \
-                if (J < 7) {                                                                              \
-                    _Pragma("unroll") for (int i = 0; i < 2; ++i)                                         \
-                        PN[i] = ld_stream4_pinned(psi + (size_t)(2 * (J + 1) + i) * NT);                  \
-                    _Pragma("unroll") for (int i = 0; i < 4; ++i)                                         \
-                        ON[i] = ldg2_pinned(obj + (size_t)(4 * (J + 1) + i) * ostride);                   \
-                }                                                                                         \
-                _Pragma("unroll") for (int i = 0; i < 4; ++i) {                                           \
-                    const float4 pp = PC[i >> 1];                                                         \
-                    const float2 ps = (i & 1) ? make_float2(pp.z, pp.w) : make_float2(pp.x, pp.y);        \
-                    if (live) red_add2(gobj + (size_t)(4 * J + i) * ostride, cmulc(ps, v[4 * J + i]));    \
-                    v[4 * J + i] = cmulc(OC[i], v[4 * J + i]);                                            \
-                }                                                                                         \
+                const float4* pp_ = psi0 + 128 * ((J) >> 3) + (size_t)(2 * ((J) & 7)) * NT;               \
+                pb[(J) % D][0] = ld_stream4_pinned(pp_);                                                  \
+                pb[(J) % D][1] = ld_stream4_pinned(pp_ + NT);                                             \
+                const float2* oo_ = obj0 + (size_t)((J) >> 3) * A.W + (size_t)(4 * ((J) & 7)) * ostride;  \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i) ob[(J) % D][i] = ldg2_pinned(oo_ + (size_t)i * ostride); \
             }
-            PTY_G2_BCHUNK(0, oa, ob, pa, pb) PTY_G2_BCHUNK(1, ob, oa, pb, pa) PTY_G2_BCHUNK(2, oa, ob, pa, pb)
-            PTY_G2_BCHUNK(3, ob, oa, pb, pa) PTY_G2_BCHUNK(4, oa, ob, pa, pb) PTY_G2_BCHUNK(5, ob, oa, pb, pa)
-            PTY_G2_BCHUNK(6, oa, ob, pa, pb) PTY_G2_BCHUNK(7, ob, oa, pb, pa)
-#undef PTY_G2_BCHUNK
+#define PTY_G2_STEP(J)                                                                                    \
+            {                                                                                             \
+                tmem_wait_ld();                                                                           \
+                if ((J) < 15) tmem_ld4(tb0 + 64u * (((J) + 1) >> 3) + 8u * (((J) + 1) & 7), gb[((J) + 1) & 1]); \
+                float2* go_ = gobj0 + (size_t)((J) >> 3) * A.W + (size_t)(4 * ((J) & 7)) * ostride;       \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i) {                                           \
+                    const float4 q_ = pb[(J) % D][i >> 1];                                                \
+                    const float2 ps = (i & 1) ? make_float2(q_.z, q_.w) : make_float2(q_.x, q_.y);        \
+                    const float2 g_ = gb[(J) & 1][i];                                                     \
+                    if (live) red_add2(go_ + (size_t)i * ostride, cmulc(ps, g_));                         \
+                    gb[(J) & 1][i] = cmulc(ob[(J) % D][i], g_);                                           \
+                }                                                                                         \
+                tmem_st4(tb0 + 64u * ((J) >> 3) + 8u * ((J) & 7), gb[(J) & 1]);                           \
+                if ((J) + D < 16) PTY_G2_ISSUE((J) + D)                                                   \
+            }
+            PTY_G2_ISSUE(0) PTY_G2_ISSUE(1) PTY_G2_ISSUE(2) PTY_G2_ISSUE(3) PTY_G2_ISSUE(4)
+            tmem_ld4(tb0, gb[0]);
+            PTY_G2_STEP(0) PTY_G2_STEP(1) PTY_G2_STEP(2) PTY_G2_STEP(3) PTY_G2_STEP(4) PTY_G2_STEP(5)
+            PTY_G2_STEP(6) PTY_G2_STEP(7) PTY_G2_STEP(8) PTY_G2_STEP(9) PTY_G2_STEP(10) PTY_G2_STEP(11)
+            PTY_G2_STEP(12) PTY_G2_STEP(13) PTY_G2_STEP(14) PTY_G2_STEP(15)
+#undef PTY_G2_STEP
+#undef PTY_G2_ISSUE
+        }
+        tmem_wait_st();
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+            const int o = 2 * c.gg + h;
+            g2_ld_own(c, o, v);
             fft32<-1, 0>(v, bg);
             g2_st_own(c, o, v);
         }
