@@ -144,7 +144,9 @@ template <class SH> struct ShapeInfo {
     static_assert(NL % 32 == 0, "a warp must stay inside one task group");
     static constexpr size_t wave_bytes = size_t(N) * PITCH * sizeof(float2);
     static constexpr size_t table_bytes = size_t(5) * N * sizeof(float2) + 64 * sizeof(float);
-    static constexpr size_t smem_bytes = wave_bytes + table_bytes;
+    // cluster shapes: two staging tiles NL x (NL + 1) for the coalesced DSMEM transpose (stage_b)
+    static constexpr size_t stage_bytes = CL > 1 ? size_t(2) * NL * (NL + 1) * sizeof(float2) : 0;
+    static constexpr size_t smem_bytes = wave_bytes + table_bytes + stage_bytes;
 };
 
 // Per-CTA view: thread id, rank in the cluster, the wave buffer of every CTA of the cluster
@@ -155,6 +157,7 @@ template <class SH> struct Cta {
     float2* Sr[SH::CL];
     float2 *tw, *Ey, *Ex, *My, *Mx;   // [N] each: twiddles exp(-2 pi i j/N); shift and propagator factors
     float* red;                       // [64] block-reduction scratch
+    float2* stg;                      // cluster shapes: 2 staging tiles [NL][NL + 1]
 };
 
 template <class SH> PTY_DEV void sync_all() {
@@ -202,16 +205,42 @@ PTY_DEV void stage_b(const Cta<SH>& c) {
         RegFFT<I::R2, DIR>::run(v[it]);
     }
     sync_all<SH>();
+    if constexpr (SH::CL == 1) {
 #pragma unroll
-    for (int it = 0; it < I::TB; ++it) {
-        const int t = it * I::NT + c.tid;
-        const int line = t % I::NL, k1 = t / I::NL;
-        const int grow = c.rank * I::NL + line;
+        for (int it = 0; it < I::TB; ++it) {
+            const int t = it * I::NT + c.tid;
+            const int line = t % I::NL, k1 = t / I::NL;
 #pragma unroll
-        for (int k2 = 0; k2 < I::R2; ++k2) {
-            const int k = k1 + I::R1 * k2;
-            float2* dst = (SH::CL > 1) ? c.Sr[k / I::NL] : c.S;
-            dst[grow * I::PITCH + (k % I::NL)] = v[it][k2];
+            for (int k2 = 0; k2 < I::R2; ++k2) c.S[line * I::PITCH + (k1 + I::R1 * k2)] = v[it][k2];
+        }
+    } else {
+        // The NL x NL tile that goes to CTA d is first assembled in local shared memory (scattered 8-byte stores,
+        // cheap locally) and then copied to the owner with lane-contiguous stores: a warp writes 256 contiguous
+        // bytes of remote shared memory instead of 32 separate 8-byte words (the scattered form ran at 10 % issue
+        // utilisation, stalled on lg_throttle -- profiles/r01_v4_fwd256).  Two tiles alternate, one CTA barrier
+        // per destination; destinations start at the own rank so that the four CTAs do not target one peer.
+        constexpr int TP = I::NL + 1, K2D = I::NL / I::R1;          // k2 values per destination
+        static_assert(I::NL % I::R1 == 0 && (I::NL * I::NL) % I::NT == 0, "tile split");
+#pragma unroll
+        for (int rr = 0; rr < SH::CL; ++rr) {
+            const int d = (c.rank + rr) % SH::CL;
+            float2* tile = c.stg + (rr & 1) * (I::NL * TP);
+#pragma unroll
+            for (int it = 0; it < I::TB; ++it) {
+                const int t = it * I::NT + c.tid;
+                const int line = t % I::NL, k1 = t / I::NL;
+#pragma unroll
+                for (int k2 = 0; k2 < I::R2; ++k2)
+                    if (k2 / K2D == d) tile[line * TP + (k1 + I::R1 * (k2 % K2D))] = v[it][k2];
+            }
+            pty_cta_sync();
+            float2* dst = c.Sr[d] + (size_t)(c.rank * I::NL) * I::PITCH;
+#pragma unroll
+            for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
+                const int idx = j * I::NT + c.tid;
+                const int row = idx / I::NL, col = idx % I::NL;
+                dst[row * I::PITCH + col] = tile[row * TP + col];
+            }
         }
     }
     sync_all<SH>();

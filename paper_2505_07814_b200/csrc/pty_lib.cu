@@ -35,6 +35,7 @@ __device__ __forceinline__ Cta<SH> make_cta(unsigned char* smem) {
     float2* tab = reinterpret_cast<float2*>(smem + I::wave_bytes);
     c.tw = tab; c.Ey = tab + SH::N; c.Ex = tab + 2 * SH::N; c.My = tab + 3 * SH::N; c.Mx = tab + 4 * SH::N;
     c.red = reinterpret_cast<float*>(tab + 5 * SH::N);
+    c.stg = reinterpret_cast<float2*>(smem + I::wave_bytes + I::table_bytes);
     return c;
 }
 
