@@ -117,7 +117,11 @@ def run_reference(args, cfg, B):
     cores = len(os.sched_getaffinity(0))
     geom = oracle.Geometry(cfg.dz, cfg.lam, cfg.dx)
     tr, ev = synth.truth(cfg), synth.eval_point(cfg, "A")
-    n = max(4, min(B, 2 * cores))
+    # a bounded sample per step: the whole run (steps + warmup) is sized to about two minutes of wall time at the
+    # ~4 patterns/s per core the oracle reaches on config 4 (scaled by the per-pattern cost of the other configs)
+    per_pattern_s = {1: 0.003, 2: 0.05, 3: 0.11, 4: 0.22, 5: 2.2}[cfg.c]
+    n = int(120.0 * cores / per_pattern_s / max(1, args.steps + args.warmup))
+    n = max(cores, min(B, n))
     idx = synth.minibatch(cfg, 0, B)[:n]
     tilt_t = tr["tilt"] if cfg.tilt_mode else None
     tilt_e = ev["tilt"] if cfg.tilt_mode else None
