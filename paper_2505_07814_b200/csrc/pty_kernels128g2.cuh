@@ -284,9 +284,10 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
         }
         tmem_wait_st();
     }
-    // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2 (through X so that the reductions into [ky][kx] are coalesced)
-    float* Xf = reinterpret_cast<float*>(c.X);
-    c.acquireX();
+    // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2.  I is kept in thread order as pairs, [r / 2][128 o + ky][r & 1]
+    // (layout K: register r of role o holds k_x = 8 o + (r & 7) + 32 (r >> 3)): one 8-byte vector RED per two
+    // registers, lane-contiguous, no transpose; pty_loss_seed128_kernel<true> reads it in that order.
+    float2* Ib = reinterpret_cast<float2*>(A.I + (size_t)b * NN);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -294,22 +295,15 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
         g2_radix4<-1>(c, o, v);
         float2* Psi = A.ws_Psi + bm * NN + 128 * o + c.c;
 #pragma unroll
-        for (int r = 0; r < 32; ++r) {
-            const float2 p = cscale(v[r], 1.0f / N);
-            if (live) st_stream2(Psi + r * NT, p);
-            Xf[c.c * P + c.kx(o, r)] = p.x * p.x + p.y * p.y;
+        for (int r = 0; r < 32; r += 2) {
+            const float2 p0 = cscale(v[r], 1.0f / N), p1 = cscale(v[r + 1], 1.0f / N);
+            if (live) {
+                st_stream2(Psi + r * NT, p0);
+                st_stream2(Psi + (r + 1) * NT, p1);
+                red_add2(Ib + (r >> 1) * NT + 128 * o + c.c, make_float2(p0.x * p0.x + p0.y * p0.y, p1.x * p1.x + p1.y * p1.y));
+            }
         }
     }
-    c.grp_sync();
-    float* Ib = A.I + (size_t)b * NN;
-    if (live) {
-#pragma unroll 8
-        for (int j = 0; j < 64; ++j) {
-            const int idx = j * 256 + c.t;
-            red_add(Ib + idx, Xf[(idx >> 7) * P + (idx & 127)]);
-        }
-    }
-    c.releaseX();
     if (c.G == 0) c.acquireX();      // consume group 1's last release
 }
 

@@ -126,8 +126,13 @@ __global__ void __launch_bounds__(F128::NT, 1) pty_probe_grad128_kernel(const fl
 // w = 2 (1 - a / sqrt(I)) / N (0 where I = 0, reading R14) written in the adjoint kernel's thread
 // order [register r = 8 (kx >> 5) + (kx & 7)][tid = 128 ((kx >> 3) & 3) + ky].  One block of 256 threads
 // per position; 32-row tiles are transposed through shared memory so that both sides are coalesced.
+// TORD: I is in the two-items-per-CTA kernels' thread order [r / 2][128 g + ky][r & 1]; the measured amplitudes are
+// transposed through the tile instead, and the natural-order copy of I (the optional `intensity` output of
+// pty_forward_loss) is written from here.
+template <bool TORD>
 __global__ void __launch_bounds__(256) pty_loss_seed128_kernel(const float* __restrict__ I, const float* __restrict__ a,
-                                                              double* loss, float* loss_per_pos, float* __restrict__ seed_w) {
+                                                              double* loss, float* loss_per_pos, float* __restrict__ seed_w,
+                                                              float* __restrict__ intensity) {
     constexpr int N = 128;
     __shared__ float tile[32][N + 1];
     __shared__ double part[8];
@@ -140,17 +145,31 @@ __global__ void __launch_bounds__(256) pty_loss_seed128_kernel(const float* __re
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             const int idx = j * 256 + t, row = idx >> 7, kx = idx & 127;
-            const float iv = __ldg(Ib + (ky0 + row) * N + kx), av = __ldg(ab + (ky0 + row) * N + kx);
-            const float d = sqrtf(iv) - av;
-            acc += d * d;
-            tile[row][kx] = iv > 1e-30f ? 2.0f * (1.0f - av * rsqrtf(iv)) * (1.0f / N) : 0.f;
+            const float av = __ldg(ab + (ky0 + row) * N + kx);
+            if (TORD) {
+                tile[row][kx] = av;
+            } else {
+                const float iv = __ldg(Ib + (ky0 + row) * N + kx);
+                const float d = sqrtf(iv) - av;
+                acc += d * d;
+                tile[row][kx] = iv > 1e-30f ? 2.0f * (1.0f - av * rsqrtf(iv)) * (1.0f / N) : 0.f;
+            }
         }
         __syncthreads();
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             const int idx = j * 256 + t, row = idx & 31, kx = idx >> 5;
             const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3;
-            Wb[r * 512 + 128 * g + ky0 + row] = tile[row][kx];
+            if (TORD) {
+                const float iv = __ldg(Ib + ((r >> 1) * 512 + 128 * g + ky0 + row) * 2 + (r & 1));
+                const float av = tile[row][kx];
+                const float d = sqrtf(iv) - av;
+                acc += d * d;
+                Wb[r * 512 + 128 * g + ky0 + row] = iv > 1e-30f ? 2.0f * (1.0f - av * rsqrtf(iv)) * (1.0f / N) : 0.f;
+                if (intensity) intensity[(size_t)b * N * N + (ky0 + row) * N + kx] = iv;
+            } else {
+                Wb[r * 512 + 128 * g + ky0 + row] = tile[row][kx];
+            }
         }
         __syncthreads();
     }
@@ -516,11 +535,13 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
                            d.tilt_mode == 1 ? tilt : (const float*)nullptr, p->at<float2>(p->L.prop), p->at<float2>(p->L.prop) + d.N));
     PTY_CUDA(p, cudaMemsetAsync(A.I, 0, (size_t)B * NN * sizeof(float), st));
     PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fwd<Shape<64>>(p, A, st), launch_fwd<Shape<128>>(p, A, st), launch_fwd<Shape<256>>(p, A, st)));
-    if (d.N == 128 && p->reg128)
-        PTY_CUDA(p, launch(p, pty_loss_seed128_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w));
+    if (d.N == 128 && p->reg128 && p->g2)
+        PTY_CUDA(p, launch(p, pty_loss_seed128_kernel<true>, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w, intensity));
+    else if (d.N == 128 && p->reg128)
+        PTY_CUDA(p, launch(p, pty_loss_seed128_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w, (float*)nullptr));
     else
         PTY_CUDA(p, launch(p, pty_loss_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)NN, loss, loss_per_pos));
-    if (intensity)
+    if (intensity && !(d.N == 128 && p->reg128 && p->g2))
         PTY_CUDA(p, cudaMemcpyAsync(intensity, A.I, (size_t)B * NN * sizeof(float), cudaMemcpyDeviceToDevice, st));
     p->fwd_valid = true;
     p->f_object = object; p->f_probe = probe; p->f_positions = positions; p->f_tilt = tilt; p->f_meas = meas;
