@@ -156,18 +156,29 @@ __global__ void __launch_bounds__(256) pty_loss_seed128_kernel(const float* __re
             }
         }
         __syncthreads();
+        if (TORD) {
+            // one thread per (ky, pair of k_x): the pair (r, r + 1) of I is one 8-byte word, lanes along ky
+            const float2* I2 = reinterpret_cast<const float2*>(Ib);
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-            const int idx = j * 256 + t, row = idx & 31, kx = idx >> 5;
-            const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3;
-            if (TORD) {
-                const float iv = __ldg(Ib + ((r >> 1) * 512 + 128 * g + ky0 + row) * 2 + (r & 1));
-                const float av = tile[row][kx];
-                const float d = sqrtf(iv) - av;
-                acc += d * d;
-                Wb[r * 512 + 128 * g + ky0 + row] = iv > 1e-30f ? 2.0f * (1.0f - av * rsqrtf(iv)) * (1.0f / N) : 0.f;
-                if (intensity) intensity[(size_t)b * N * N + (ky0 + row) * N + kx] = iv;
-            } else {
+            for (int j = 0; j < 8; ++j) {
+                const int idx = j * 256 + t, row = idx & 31, kx = 2 * (idx >> 5);
+                const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3, ky = ky0 + row;
+                const float2 iv = __ldg(I2 + (r >> 1) * 512 + 128 * g + ky);
+                const float a0 = tile[row][kx], a1 = tile[row][kx + 1];
+                const float d0 = sqrtf(iv.x) - a0, d1 = sqrtf(iv.y) - a1;
+                acc += d0 * d0 + d1 * d1;
+                Wb[r * 512 + 128 * g + ky] = iv.x > 1e-30f ? 2.0f * (1.0f - a0 * rsqrtf(iv.x)) * (1.0f / N) : 0.f;
+                Wb[(r + 1) * 512 + 128 * g + ky] = iv.y > 1e-30f ? 2.0f * (1.0f - a1 * rsqrtf(iv.y)) * (1.0f / N) : 0.f;
+                if (intensity) {
+                    float* o = intensity + (size_t)b * N * N + ky * N + kx;
+                    o[0] = iv.x; o[1] = iv.y;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const int idx = j * 256 + t, row = idx & 31, kx = idx >> 5;
+                const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3;
                 Wb[r * 512 + 128 * g + ky0 + row] = tile[row][kx];
             }
         }
