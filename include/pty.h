@@ -21,6 +21,14 @@
  * DC at index [0][0] (unshifted FFT order).  positions[b] = (p_y, p_x) in PIXELS = the top-left
  * corner of the N x N crop in object coordinates.  tilt = (theta_y, theta_x) in RADIANS.
  *
+ * Alignment.  object, probe and every complex gradient: 8 bytes; meas_amp: 16 bytes; positions,
+ * tilt and the real gradients: 4 bytes (violations return PTY_ERR_INVALID_ARG).  The Adam arrays
+ * (theta, grad, m, v) may have any 4-byte alignment: the update uses 16-byte vectors when all four
+ * are 16-byte aligned and a scalar path otherwise (e.g. a positions[lo:hi] shard view).
+ *
+ * Devices.  A plan belongs to the device given to pty_create.  Every entry point switches to that
+ * device for its own duration and restores the caller's current device before it returns.
+ *
  * Memory.  Unless a parameter says "host", every pointer is a DEVICE pointer on the plan's
  * device.  The caller owns every buffer including the workspace and the Adam moments; the
  * library allocates no device memory, frees nothing of the caller's and keeps no caller pointer
@@ -60,7 +68,11 @@ extern "C" {
 
 /* pty_backward flags */
 #define PTY_BWD_ACCUMULATE     1    /* add into the gradient outputs instead of overwriting    */
-#define PTY_BWD_RECOMPUTE      2    /* do not trust the state left by pty_forward_loss         */
+#define PTY_BWD_REUSE_FORWARD  4    /* the caller asserts that object, probe, positions, tilt and
+                                       meas_amp are BIT-UNCHANGED since the pty_forward_loss call
+                                       made just before on this plan and stream with the same
+                                       pointers and B: its saved waves are reused.  Without this
+                                       flag pty_backward always runs the forward itself.        */
 
 typedef struct pty_plan pty_plan;   /* opaque, host side */
 
@@ -113,15 +125,17 @@ int pty_forward_loss(pty_plan* plan, const void* object, const void* probe,
                      double* loss, float* loss_per_pos, float* intensity, void* stream);
 
 /* Exact gradient of L for the same minibatch (hand-written adjoint).
- * Uses the state left by the immediately preceding pty_forward_loss on this plan when that call
- * had the same pointers and B; otherwise (or with PTY_BWD_RECOMPUTE) it runs the forward itself.
+ * Runs the forward itself unless flags has PTY_BWD_REUSE_FORWARD, which reuses the waves saved by
+ * the immediately preceding pty_forward_loss (same plan, stream, pointers and B).  Reuse is by
+ * pointer identity only: with that flag the caller guarantees the arrays were not modified in
+ * between (any pty_step / pty_adam_update on the plan cancels the saved state by itself).
  * Outputs (device; any may be NULL = not wanted, except g_object):
  *   g_object    [Nz][H][W] c64  scatter-add over the overlapping patches
  *   g_probe     [M][N][N] c64
  *   g_positions [B][2] f32      = dL/dDelta_b  (y, x)
  *   g_tilt      [2] (tilt_mode 1: summed over b) or [B][2] (tilt_mode 2); ignored for mode 0
  *   g_dz        [1] f32         = dL/d(dz); needs tilt_mode != 0 or PTY_FLAG_SPECTRA
- * flags: PTY_BWD_ACCUMULATE, PTY_BWD_RECOMPUTE. */
+ * flags: PTY_BWD_ACCUMULATE, PTY_BWD_REUSE_FORWARD. */
 int pty_backward(pty_plan* plan, const void* object, const void* probe,
                  const float* positions, const float* tilt, const float* meas_amp, int32_t B,
                  void* g_object, void* g_probe, float* g_positions, float* g_tilt, float* g_dz,
@@ -153,8 +167,8 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe,
 int pty_status(pty_plan* plan, int32_t* device_flags);
 
 /* Kernel timing for benchmarks.  pty_profile(plan, 1) makes every later call bracket its forward
- * (a2-a5) and adjoint (a7-a13) kernel launches with CUDA events on the call's own stream (at most
- * 1024 launches are kept; older ones are dropped); pty_profile(plan, 0) stops and forgets them.
+ * (a2-a5) and adjoint (a7-a13) kernel launches with CUDA events on the call's own stream (the first
+ * 1024 launches after enabling are kept; later ones are not recorded until the next read); pty_profile(plan, 0) stops and forgets them.
  * pty_profile_read synchronises the plan's stream and returns, for the launches recorded since the
  * last read, the summed device time in milliseconds and the launch count of each kernel (host out). */
 int pty_profile(pty_plan* plan, int32_t enable);
@@ -166,14 +180,7 @@ int64_t pty_launch_count(const pty_plan* plan);
 /* Text of the plan's last error ("" if none).  plan == NULL returns the last creation error. */
 const char* pty_last_error(const pty_plan* plan);
 
-/* Library version string, e.g. "pty-b200 0.1 (sm_100a)". */
-/* FP32 pipe microbenchmark ("measure an FMA microbenchmark peak and the clock actually held"):
- * runs a kernel of independent scalar FFMA chains (packed = 0) or packed FFMA2 chains (packed = 1) on every SM of
- * `device` for about 20 ms and writes the achieved TFLOP/s (2 flops per FMA lane-operation) to *tflops (host).
- * Allocates and frees 4 bytes of device memory; synchronises the device.  Not part of the hot path: bench.py
- * reports it beside the nominal peak.  Returns PTY_OK or PTY_ERR_CUDA / PTY_ERR_INVALID_ARG. */
-int pty_fma_peak(int32_t device, int32_t packed, double* tflops);
-
+/* Library version string, e.g. "pty-b200 0.2 (sm_100a)". */
 const char* pty_version(void);
 
 #ifdef __cplusplus

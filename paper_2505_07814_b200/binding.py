@@ -24,11 +24,11 @@ lib = C.CDLL(LIB_PATH)
 PTY_OK, PTY_ERR_INVALID_ARG, PTY_ERR_UNSUPPORTED = 0, -1, -2
 PTY_ERR_WORKSPACE, PTY_ERR_CUDA, PTY_ERR_BOUNDS = -3, -4, -5
 PTY_FLAG_SPECTRA, PTY_FLAG_STEP, PTY_FLAG_HOST = 1, 2, 4
-PTY_BWD_ACCUMULATE, PTY_BWD_RECOMPUTE = 1, 2
+PTY_BWD_ACCUMULATE, PTY_BWD_REUSE_FORWARD = 1, 4
 
 EXPORTS = ["pty_workspace_bytes", "pty_create", "pty_destroy", "pty_forward_loss", "pty_backward",
            "pty_step", "pty_adam_update", "pty_grad_host", "pty_status", "pty_profile",
-           "pty_profile_read", "pty_launch_count", "pty_last_error", "pty_version", "pty_fma_peak"]
+           "pty_profile_read", "pty_launch_count", "pty_last_error", "pty_version"]
 
 
 class pty_dims(C.Structure):
@@ -68,7 +68,6 @@ lib.pty_launch_count.restype = C.c_int64
 lib.pty_last_error.argtypes = [_vp]
 lib.pty_last_error.restype = C.c_char_p
 lib.pty_version.restype = C.c_char_p
-lib.pty_fma_peak.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double)]
 for _n in EXPORTS[:11]:
     getattr(lib, _n).restype = C.c_int
 
@@ -201,12 +200,3 @@ def plan_for(cfg, Bmax=None, flags=0, device=0):
     """Plan for a ``synth.Config``."""
     return Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, cfg.B if Bmax is None else Bmax, cfg.dz, cfg.lam, cfg.dx,
                 tilt_mode=cfg.tilt_mode, flags=flags, device=device)
-
-
-def fma_peak(device=0, packed=False):
-    """FP32 FMA microbenchmark on `device` (include/pty.h: pty_fma_peak): achieved TFLOP/s."""
-    out = C.c_double(0.0)
-    rc = lib.pty_fma_peak(int(device), 1 if packed else 0, C.byref(out))
-    if rc != 0:
-        raise RuntimeError(f"pty_fma_peak failed: {rc}")
-    return out.value

@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(SH::NT, MinBlocks<SH>::value) pty_bwd_kernel(c
     bwd_body<SH>(A, c, blockIdx.x / SH::CL);
 }
 
-// N = 128 on the register-resident FFT (pty_fft128.cuh): the default path for the headline config
+// N = 128 helpers on the one-item register-resident FFT (pty_fft128.cuh): probe spectrum and probe gradient
 __device__ __forceinline__ Cta128 make_cta128(unsigned char* smem) {
     Cta128 c;
     c.tid = threadIdx.x;
@@ -80,18 +80,6 @@ __device__ __forceinline__ void release_cta128(unsigned char* smem) {
     __syncthreads();
     float2* tab = reinterpret_cast<float2*>(smem + F128::xch_bytes);
     if ((threadIdx.x >> 5) == 0) tmem_dealloc512(*reinterpret_cast<unsigned*>(reinterpret_cast<float*>(tab + 640) + 64));
-}
-
-__global__ void __launch_bounds__(F128::NT, 1) pty_fwd128_kernel(const KArgs A) {
-    extern __shared__ __align__(16) unsigned char smem[];
-    fwd_body128(A, make_cta128(smem), blockIdx.x);
-    release_cta128(smem);
-}
-
-__global__ void __launch_bounds__(F128::NT, 1) pty_bwd128_kernel(const KArgs A) {
-    extern __shared__ __align__(16) unsigned char smem[];
-    bwd_body128(A, make_cta128(smem), blockIdx.x);
-    release_cta128(smem);
 }
 
 // N = 128, two items per CTA (pty_kernels128g2.cuh): group G of CTA x owns item 2 x + G
@@ -122,14 +110,12 @@ __global__ void __launch_bounds__(F128::NT, 1) pty_probe_grad128_kernel(const fl
     release_cta128(smem);
 }
 
-// a6 + a7 for the N = 128 register path: L_b = sum_k (sqrt(I_b) - a_b)^2 and the seed weights
-// w = 2 (1 - a / sqrt(I)) / N (0 where I = 0, reading R14) written in the adjoint kernel's thread
-// order [register r = 8 (kx >> 5) + (kx & 7)][tid = 128 ((kx >> 3) & 3) + ky].  One block of 256 threads
-// per position; 32-row tiles are transposed through shared memory so that both sides are coalesced.
-// TORD: I is in the two-items-per-CTA kernels' thread order [r / 2][128 g + ky][r & 1]; the measured amplitudes are
-// transposed through the tile instead, and the natural-order copy of I (the optional `intensity` output of
-// pty_forward_loss) is written from here.
-template <bool TORD>
+// a6 + a7 for N = 128: L_b = sum_k (sqrt(I_b) - a_b)^2 and the seed weights w = 2 (1 - a / sqrt(I)) / N
+// (0 where I = 0, reading R14) written in the adjoint kernel's thread order
+// [register r = 8 (kx >> 5) + (kx & 7)][tid = 128 ((kx >> 3) & 3) + ky].  I arrives in the forward kernel's thread
+// order as pairs, [r / 2][128 o + ky][r & 1]; the measured amplitudes (natural order) are transposed through a
+// 32-row shared tile so that both sides are coalesced; the natural-order copy of I (the optional `intensity`
+// output of pty_forward_loss) is written from here.  One block of 256 threads per position.
 __global__ void __launch_bounds__(256) pty_loss_seed128_kernel(const float* __restrict__ I, const float* __restrict__ a,
                                                               double* loss, float* loss_per_pos, float* __restrict__ seed_w,
                                                               float* __restrict__ intensity) {
@@ -137,7 +123,7 @@ __global__ void __launch_bounds__(256) pty_loss_seed128_kernel(const float* __re
     __shared__ float tile[32][N + 1];
     __shared__ double part[8];
     const int b = blockIdx.x, t = threadIdx.x;
-    const float* Ib = I + (size_t)b * N * N;
+    const float2* I2 = reinterpret_cast<const float2*>(I + (size_t)b * N * N);
     const float* ab = a + (size_t)b * N * N;
     float* Wb = seed_w + (size_t)b * N * N;
     float acc = 0.f;
@@ -145,41 +131,23 @@ __global__ void __launch_bounds__(256) pty_loss_seed128_kernel(const float* __re
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             const int idx = j * 256 + t, row = idx >> 7, kx = idx & 127;
-            const float av = __ldg(ab + (ky0 + row) * N + kx);
-            if (TORD) {
-                tile[row][kx] = av;
-            } else {
-                const float iv = __ldg(Ib + (ky0 + row) * N + kx);
-                const float d = sqrtf(iv) - av;
-                acc += d * d;
-                tile[row][kx] = iv > 1e-30f ? 2.0f * (1.0f - av * rsqrtf(iv)) * (1.0f / N) : 0.f;
-            }
+            tile[row][kx] = __ldg(ab + (ky0 + row) * N + kx);
         }
         __syncthreads();
-        if (TORD) {
-            // one thread per (ky, pair of k_x): the pair (r, r + 1) of I is one 8-byte word, lanes along ky
-            const float2* I2 = reinterpret_cast<const float2*>(Ib);
+        // one thread per (ky, pair of k_x): the pair (r, r + 1) of I is one 8-byte word, lanes along ky
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const int idx = j * 256 + t, row = idx & 31, kx = 2 * (idx >> 5);
-                const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3, ky = ky0 + row;
-                const float2 iv = __ldg(I2 + (r >> 1) * 512 + 128 * g + ky);
-                const float a0 = tile[row][kx], a1 = tile[row][kx + 1];
-                const float d0 = sqrtf(iv.x) - a0, d1 = sqrtf(iv.y) - a1;
-                acc += d0 * d0 + d1 * d1;
-                Wb[r * 512 + 128 * g + ky] = iv.x > 1e-30f ? 2.0f * (1.0f - a0 * rsqrtf(iv.x)) * (1.0f / N) : 0.f;
-                Wb[(r + 1) * 512 + 128 * g + ky] = iv.y > 1e-30f ? 2.0f * (1.0f - a1 * rsqrtf(iv.y)) * (1.0f / N) : 0.f;
-                if (intensity) {
-                    float* o = intensity + (size_t)b * N * N + ky * N + kx;
-                    o[0] = iv.x; o[1] = iv.y;
-                }
-            }
-        } else {
-#pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                const int idx = j * 256 + t, row = idx & 31, kx = idx >> 5;
-                const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3;
-                Wb[r * 512 + 128 * g + ky0 + row] = tile[row][kx];
+        for (int j = 0; j < 8; ++j) {
+            const int idx = j * 256 + t, row = idx & 31, kx = 2 * (idx >> 5);
+            const int r = 8 * (kx >> 5) + (kx & 7), g = (kx >> 3) & 3, ky = ky0 + row;
+            const float2 iv = __ldg(I2 + (r >> 1) * 512 + 128 * g + ky);
+            const float a0 = tile[row][kx], a1 = tile[row][kx + 1];
+            const float d0 = sqrtf(iv.x) - a0, d1 = sqrtf(iv.y) - a1;
+            acc += d0 * d0 + d1 * d1;
+            Wb[r * 512 + 128 * g + ky] = iv.x > 1e-30f ? 2.0f * (1.0f - a0 * rsqrtf(iv.x)) * (1.0f / N) : 0.f;
+            Wb[(r + 1) * 512 + 128 * g + ky] = iv.y > 1e-30f ? 2.0f * (1.0f - a1 * rsqrtf(iv.y)) * (1.0f / N) : 0.f;
+            if (intensity) {
+                float* o = intensity + (size_t)b * N * N + ky * N + kx;
+                o[0] = iv.x; o[1] = iv.y;
             }
         }
         __syncthreads();
@@ -251,14 +219,15 @@ __global__ void __launch_bounds__(256) pty_loss_kernel(const float* __restrict__
     }
 }
 
-// a13 (B8): tilt and dz gradients from the per-position sums of D(k) (k in cycles/pixel).
-__global__ void pty_tilt_finalize_kernel(const float* dsum, const float* tilt, int B, int tilt_mode,
-                                         float dz, float lambda, float dx, float* g_tilt, float* g_dz,
-                                         int accumulate) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+// a13 (B8): tilt and dz gradients from the per-position sums of D(k) (k in cycles/pixel).  One block; thread t
+// handles positions t, t + 256, ...; the sums over b (global tilt, dz) are reduced in double precision.
+__global__ void __launch_bounds__(256) pty_tilt_finalize_kernel(const float* dsum, const float* tilt, int B, int tilt_mode,
+                                                                 float dz, float lambda, float dx, float* g_tilt, float* g_dz,
+                                                                 int accumulate) {
     const double two_pi = 6.283185307179586476925;
+    __shared__ double part[3][8];
     double gty = 0.0, gtx = 0.0, gz = 0.0;
-    for (int b = 0; b < B; ++b) {
+    for (int b = threadIdx.x; b < B; b += blockDim.x) {
         double ty = 0.0, tx = 0.0;
         if (tilt_mode == 1) { ty = tilt[0]; tx = tilt[1]; }
         if (tilt_mode == 2) { ty = tilt[2 * b]; tx = tilt[2 * b + 1]; }
@@ -273,6 +242,19 @@ __global__ void pty_tilt_finalize_kernel(const float* dsum, const float* tilt, i
         }
         gty += ay; gtx += ax;
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        gty += __shfl_xor_sync(0xffffffffu, gty, o);
+        gtx += __shfl_xor_sync(0xffffffffu, gtx, o);
+        gz += __shfl_xor_sync(0xffffffffu, gz, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        part[0][threadIdx.x >> 5] = gty; part[1][threadIdx.x >> 5] = gtx; part[2][threadIdx.x >> 5] = gz;
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    gty = gtx = gz = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { gty += part[0][w]; gtx += part[1][w]; gz += part[2][w]; }
     if (tilt_mode == 1 && g_tilt) {
         g_tilt[0] = (accumulate ? g_tilt[0] : 0.f) + (float)gty;
         g_tilt[1] = (accumulate ? g_tilt[1] : 0.f) + (float)gtx;
@@ -283,10 +265,10 @@ __global__ void pty_tilt_finalize_kernel(const float* dsum, const float* tilt, i
 // a14 (B9): bias-corrected Adam on a flat float array.  HBM-bound: streams theta, g, m, v.
 __global__ void __launch_bounds__(256) pty_adam_kernel(float* __restrict__ theta, const float* __restrict__ g,
                                                        float* __restrict__ m, float* __restrict__ v, size_t n,
-                                                       float lr, float b1, float b2, float omb1, float omb2,
+                                                       size_t n4, float lr, float b1, float b2, float omb1, float omb2,
                                                        float eps, float inv_bc1, float inv_bc2) {
+    // n4 = number of leading float4 groups (n / 4, or 0 when some array is not 16-byte aligned: scalar path)
     const size_t stride = (size_t)gridDim.x * blockDim.x;
-    const size_t n4 = n / 4;
     float4* t4 = reinterpret_cast<float4*>(theta);
     const float4* g4 = reinterpret_cast<const float4*>(g);
     float4* m4 = reinterpret_cast<float4*>(m);
@@ -382,8 +364,6 @@ struct pty_plan {
     const void *f_object, *f_probe, *f_positions, *f_tilt, *f_meas;
     int32_t f_B;
 
-    bool g2;                     // N = 128: two items per CTA (pty_kernels128g2.cuh)
-    bool reg128;                 // N = 128 on the register-resident FFT (default) or the shared-memory passes
     // optional kernel timing (pty_profile)
     bool profiling;
     struct Timed { cudaEvent_t a, b; int which; };
@@ -406,6 +386,15 @@ int fail(pty_plan* p, int code, const char* fmt, ...) {
     if (p) p->err = buf; else g_create_error = buf;
     return code;
 }
+
+// Every entry point runs on the plan's device whatever the caller's current device is, and restores it.
+struct DeviceGuard {
+    int prev; bool switched;
+    explicit DeviceGuard(int device) : prev(-1), switched(false) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 #define PTY_CUDA(p, call)                                                                     \
     do {                                                                                      \
@@ -469,25 +458,28 @@ struct ScopedTimer {
     }
 };
 
-template <class SH> cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
-    ScopedTimer tm(p, 0, st);
-    if (SH::N == 128 && p->reg128 && p->g2)
-        return launch(p, pty_fwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
-    if (SH::N == 128 && p->reg128)
-        return launch(p, pty_fwd128_kernel, A.B * A.M, F128::NT, F128::smem_bytes, 1, st, A);
+// N = 128 runs the two-items-per-CTA kernels (pty_kernels128g2.cuh); N = 64 and N = 256 the shared-memory passes
+template <class SH> cudaError_t launch_fwd_sh(pty_plan* p, const KArgs& A, cudaStream_t st) {
     return launch(p, pty_fwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
-template <class SH> cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
-    ScopedTimer tm(p, 1, st);
-    if (SH::N == 128 && p->reg128 && p->g2)
-        return launch(p, pty_bwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
-    if (SH::N == 128 && p->reg128)
-        return launch(p, pty_bwd128_kernel, A.B * A.M, F128::NT, F128::smem_bytes, 1, st, A);
+template <class SH> cudaError_t launch_bwd_sh(pty_plan* p, const KArgs& A, cudaStream_t st) {
     return launch(p, pty_bwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
-
-#define PTY_DISPATCH_N(p, expr64, expr128, expr256)                     \
-    ((p)->d.N == 64 ? (expr64) : (p)->d.N == 128 ? (expr128) : (expr256))
+cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
+    ScopedTimer tm(p, 0, st);
+    if (p->d.N == 128) return launch(p, pty_fwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
+    return p->d.N == 64 ? launch_fwd_sh<Shape<64>>(p, A, st) : launch_fwd_sh<Shape<256>>(p, A, st);
+}
+cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
+    ScopedTimer tm(p, 1, st);
+    if (p->d.N == 128) return launch(p, pty_bwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
+    return p->d.N == 64 ? launch_bwd_sh<Shape<64>>(p, A, st) : launch_bwd_sh<Shape<256>>(p, A, st);
+}
+// plain 2-D FFT of `items` planes (N = 64, 256): P^ = F[P] / N and g_probe = F^-1[G^_P] / N
+cudaError_t launch_fft2_n(pty_plan* p, int dir, const float2* src, float2* dst, float scale, int acc, int items, cudaStream_t st) {
+    return p->d.N == 64 ? launch_fft2<Shape<64>>(p, dir, src, dst, scale, acc, items, st)
+                        : launch_fft2<Shape<256>>(p, dir, src, dst, scale, acc, items, st);
+}
 
 KArgs make_args(const pty_plan* p, const void* object, const float* positions, const float* tilt,
                 const float* meas, int32_t B) {
@@ -521,6 +513,13 @@ int check_batch(pty_plan* p, const void* object, const void* probe, const float*
     if (!object || !probe || (B > 0 && (!positions || !meas))) return fail(p, PTY_ERR_INVALID_ARG, "null input pointer");
     if (p->d.tilt_mode != 0 && !tilt) return fail(p, PTY_ERR_INVALID_ARG, "tilt_mode %d needs a tilt pointer", p->d.tilt_mode);
     if (B < 0 || B > p->d.Bmax) return fail(p, PTY_ERR_INVALID_ARG, "B = %d outside [0, Bmax = %d]", B, p->d.Bmax);
+    // complex arrays are read as 8-byte words, the measured amplitudes as 16-byte vectors (pty.h "Alignment")
+    if ((reinterpret_cast<uintptr_t>(object) & 7) || (reinterpret_cast<uintptr_t>(probe) & 7))
+        return fail(p, PTY_ERR_INVALID_ARG, "object and probe must be 8-byte aligned");
+    if (reinterpret_cast<uintptr_t>(meas) & 15)
+        return fail(p, PTY_ERR_INVALID_ARG, "meas_amp must be 16-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(positions) & 3) || (reinterpret_cast<uintptr_t>(tilt) & 3))
+        return fail(p, PTY_ERR_INVALID_ARG, "positions and tilt must be 4-byte aligned");
     return PTY_OK;
 }
 
@@ -535,24 +534,20 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
     if (B == 0) return PTY_OK;
     KArgs A = make_args(p, object, positions, tilt, meas, B);
     // a0: probe spectrum (unitary) and propagator factors
-    if (d.N == 128 && p->reg128)
+    if (d.N == 128)
         PTY_CUDA(p, launch(p, pty_probe_hat128_kernel, d.M, F128::NT, F128::smem_bytes, 1, st, (const float2*)probe, p->at<float2>(p->L.probe_hat)));
     else
-        PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fft2<Shape<64>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
-                                   launch_fft2<Shape<128>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st),
-                                   launch_fft2<Shape<256>>(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st)));
+        PTY_CUDA(p, launch_fft2_n(p, -1, (const float2*)probe, p->at<float2>(p->L.probe_hat), 1.f / d.N, 0, d.M, st));
     if (d.tilt_mode != 2)
         PTY_CUDA(p, launch(p, pty_prop_table_kernel, (d.N + 127) / 128, 128, 0, 1, st, (int)d.N, d.dz, d.lambda, d.dx,
                            d.tilt_mode == 1 ? tilt : (const float*)nullptr, p->at<float2>(p->L.prop), p->at<float2>(p->L.prop) + d.N));
     PTY_CUDA(p, cudaMemsetAsync(A.I, 0, (size_t)B * NN * sizeof(float), st));
-    PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fwd<Shape<64>>(p, A, st), launch_fwd<Shape<128>>(p, A, st), launch_fwd<Shape<256>>(p, A, st)));
-    if (d.N == 128 && p->reg128 && p->g2)
-        PTY_CUDA(p, launch(p, pty_loss_seed128_kernel<true>, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w, intensity));
-    else if (d.N == 128 && p->reg128)
-        PTY_CUDA(p, launch(p, pty_loss_seed128_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w, (float*)nullptr));
+    PTY_CUDA(p, launch_fwd(p, A, st));
+    if (d.N == 128)
+        PTY_CUDA(p, launch(p, pty_loss_seed128_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w, intensity));
     else
         PTY_CUDA(p, launch(p, pty_loss_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)NN, loss, loss_per_pos));
-    if (intensity && !(d.N == 128 && p->reg128 && p->g2))
+    if (intensity && d.N != 128)
         PTY_CUDA(p, cudaMemcpyAsync(intensity, A.I, (size_t)B * NN * sizeof(float), cudaMemcpyDeviceToDevice, st));
     p->fwd_valid = true;
     p->f_object = object; p->f_probe = probe; p->f_positions = positions; p->f_tilt = tilt; p->f_meas = meas;
@@ -578,17 +573,15 @@ int run_backward(pty_plan* p, const void* object, const float* positions, const 
     PTY_CUDA(p, cudaMemsetAsync(A.GP_hat, 0, (size_t)d.M * NN * sizeof(float2), st));
     if (A.save_hat && B) PTY_CUDA(p, cudaMemsetAsync(A.dsum, 0, (size_t)B * 4 * sizeof(float), st));
     if (B)
-        PTY_CUDA(p, PTY_DISPATCH_N(p, launch_bwd<Shape<64>>(p, A, st), launch_bwd<Shape<128>>(p, A, st), launch_bwd<Shape<256>>(p, A, st)));
-    if (want_probe && d.N == 128 && p->reg128)
+        PTY_CUDA(p, launch_bwd(p, A, st));
+    if (want_probe && d.N == 128)
         PTY_CUDA(p, launch(p, pty_probe_grad128_kernel, d.M, F128::NT, F128::smem_bytes, 1, st, (const float2*)A.GP_hat, (float2*)g_probe, (int)accumulate));
     else if (want_probe)
-        PTY_CUDA(p, PTY_DISPATCH_N(p, launch_fft2<Shape<64>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st),
-                                   launch_fft2<Shape<128>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st),
-                                   launch_fft2<Shape<256>>(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st)));
+        PTY_CUDA(p, launch_fft2_n(p, +1, A.GP_hat, (float2*)g_probe, 1.f / d.N, accumulate, d.M, st));
     const bool want_tilt = g_tilt && d.tilt_mode != 0;
     if (want_tilt || g_dz) {
         if (A.save_hat) {
-            PTY_CUDA(p, launch(p, pty_tilt_finalize_kernel, 1, 32, 0, 1, st, (const float*)A.dsum, tilt, (int)B, (int)d.tilt_mode,
+            PTY_CUDA(p, launch(p, pty_tilt_finalize_kernel, 1, 256, 0, 1, st, (const float*)A.dsum, tilt, (int)B, (int)d.tilt_mode,
                                d.dz, d.lambda, d.dx, want_tilt ? g_tilt : (float*)nullptr, g_dz, accumulate));
         } else if (!accumulate) {   // Nz == 1: no propagation, so both gradients are exactly zero
             if (want_tilt) PTY_CUDA(p, cudaMemsetAsync(g_tilt, 0, (d.tilt_mode == 2 ? (size_t)B * 2 : 2) * sizeof(float), st));
@@ -605,12 +598,15 @@ int adam_launch(pty_plan* p, float* theta, const float* g, float* m, float* v, s
     if (t < 1) return fail(p, PTY_ERR_INVALID_ARG, "adam: step number t must be >= 1");
     const float inv_bc1 = (float)(1.0 / (1.0 - pow((double)b1, (double)t)));
     const float inv_bc2 = (float)(1.0 / (1.0 - pow((double)b2, (double)t)));
-    size_t blocks = (n / 4 + 255) / 256;
+    const bool aligned = ((reinterpret_cast<uintptr_t>(theta) | reinterpret_cast<uintptr_t>(g) |
+                           reinterpret_cast<uintptr_t>(m) | reinterpret_cast<uintptr_t>(v)) & 15) == 0;
+    const size_t n4 = aligned ? n / 4 : 0;      // e.g. a positions[lo:hi] view with odd lo: scalar path
+    size_t blocks = ((aligned ? n / 4 : n) + 255) / 256;
     const size_t cap = (size_t)p->num_sms * 16;
     if (blocks > cap) blocks = cap;
     if (blocks == 0) blocks = 1;
     const float omb1 = (float)(1.0 - (double)b1), omb2 = (float)(1.0 - (double)b2);   // 1 - beta rounded once
-    PTY_CUDA(p, launch(p, pty_adam_kernel, (int)blocks, 256, 0, 1, st, theta, g, m, v, n, lr, b1, b2, omb1, omb2, eps,
+    PTY_CUDA(p, launch(p, pty_adam_kernel, (int)blocks, 256, 0, 1, st, theta, g, m, v, n, n4, lr, b1, b2, omb1, omb2, eps,
                        inv_bc1, inv_bc2));
     return PTY_OK;
 }
@@ -618,53 +614,9 @@ int adam_launch(pty_plan* p, float* theta, const float* g, float* m, float* v, s
 }  // namespace
 
 // ============================================================================ C ABI
-// FP32 pipe microbenchmark: 16 independent chains per thread, 1024 iterations, 8 CTAs of 512 threads per SM
-template <int PACKED> __global__ void __launch_bounds__(512) pty_fma_peak_kernel(float* out, float a, float b, int iters) {
-    float2 x[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) x[i] = make_float2(threadIdx.x * 1e-3f + i, i * 0.5f);
-    const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
-#pragma unroll 1
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            if (PACKED) x[i] = __ffma2_rn(x[i], a2, b2);
-            else { x[i].x = fmaf(x[i].x, a, b); x[i].y = fmaf(x[i].y, a, b); }
-        }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) s += x[i].x + x[i].y;
-    if (s == 12345.678f) out[0] = s;
-}
-
 extern "C" {
 
-int pty_fma_peak(int32_t device, int32_t packed, double* tflops) {
-    if (!tflops) return PTY_ERR_INVALID_ARG;
-    cudaDeviceProp prop;
-    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) return PTY_ERR_CUDA;
-    float* d = nullptr;
-    if (cudaMalloc(&d, 4) != cudaSuccess) return PTY_ERR_CUDA;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    const int grid = prop.multiProcessorCount * 8, iters = 1 << 16;
-    float best = 1e30f;
-    for (int r = 0; r < 3; ++r) {
-        cudaEventRecord(e0);
-        if (packed) pty_fma_peak_kernel<1><<<grid, 512>>>(d, 1.0001f, 0.5f, iters);
-        else pty_fma_peak_kernel<0><<<grid, 512>>>(d, 1.0001f, 0.5f, iters);
-        cudaEventRecord(e1);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return PTY_ERR_CUDA; }
-        float ms; cudaEventElapsedTime(&ms, e0, e1);
-        if (r && ms < best) best = ms;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
-    *tflops = 2.0 * 16.0 * (double)iters * 512.0 * grid / (best * 1e-3) / 1e12;
-    return PTY_OK;
-}
-
-const char* pty_version(void) { return "pty-b200 0.1 (sm_100a)"; }
+const char* pty_version(void) { return "pty-b200 0.2 (sm_100a)"; }
 
 int pty_workspace_bytes(const pty_dims* dims, size_t* out_bytes) {
     std::string err;
@@ -688,34 +640,29 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
     if (!p) return fail(nullptr, PTY_ERR_INVALID_ARG, "out of host memory");
     p->d = *dims; p->L = L; p->ws = static_cast<unsigned char*>(workspace); p->device = device;
     p->last_stream = nullptr; p->launches = 0; p->fwd_valid = false; p->profiling = false;
-    cudaError_t e = cudaSetDevice(device);
+    int prev_device = -1;
+    cudaError_t e = cudaGetDevice(&prev_device);
+    if (e == cudaSuccess) e = cudaSetDevice(device);
     cudaDeviceProp prop{};
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
-    if (e == cudaSuccess && prop.major < 10) {
+    if (e == cudaSuccess && !(prop.major == 10 && prop.minor == 0)) {
         delete p;
-        return fail(nullptr, PTY_ERR_UNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor);
+        cudaSetDevice(prev_device);
+        return fail(nullptr, PTY_ERR_UNSUPPORTED, "device %d is sm_%d%d; this library holds sm_100a code only", device, prop.major, prop.minor);
     }
-    if (e == cudaSuccess) e = PTY_DISPATCH_N(p, set_smem_attrs<Shape<64>>(), set_smem_attrs<Shape<128>>(), set_smem_attrs<Shape<256>>());
-    // N = 128 kernel family: default = two items per CTA (pty_kernels128g2.cuh); PTY_FFT128=reg selects the
-    // one-item register-resident kernels (pty_kernels128.cuh), PTY_FFT128=smem the shared-memory-pass kernels
-    const char* sel = getenv("PTY_FFT128");
-    p->reg128 = !(sel && strcmp(sel, "smem") == 0);
-    p->g2 = p->reg128 && !(sel && strcmp(sel, "reg") == 0);
+    if (e == cudaSuccess && dims->N == 64) e = set_smem_attrs<Shape<64>>();
+    if (e == cudaSuccess && dims->N == 256) e = set_smem_attrs<Shape<256>>();
     if (e == cudaSuccess && dims->N == 128) {
         e = cudaFuncSetAttribute(pty_fwd128g2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_bwd128g2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
-    }
-    if (e == cudaSuccess && dims->N == 128) {
-        e = cudaFuncSetAttribute(pty_fwd128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(pty_bwd128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_probe_hat128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_probe_grad128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
     }
     if (e == cudaSuccess) e = cudaMemset(p->ws + L.scalars, 0, 256);
+    if (prev_device >= 0 && prev_device != device) cudaSetDevice(prev_device);   // leave the caller's device as it was
     if (e != cudaSuccess) {
         delete p;
         return fail(nullptr, PTY_ERR_CUDA, "pty_create: %s", cudaGetErrorString(e));
@@ -745,6 +692,7 @@ int pty_profile(pty_plan* plan, int32_t enable) {
 
 int pty_profile_read(pty_plan* plan, float* fwd_ms, int32_t* fwd_launches, float* bwd_ms, int32_t* bwd_launches) {
     if (!plan) return PTY_ERR_INVALID_ARG;
+    DeviceGuard dg(plan->device);
     PTY_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
     float ms[2] = {0.f, 0.f};
     int32_t n[2] = {0, 0};
@@ -766,6 +714,7 @@ int pty_forward_loss(pty_plan* plan, const void* object, const void* probe, cons
                      const float* meas_amp, int32_t B, double* loss, float* loss_per_pos, float* intensity, void* stream) {
     int rc = check_batch(plan, object, probe, positions, tilt, meas_amp, B);
     if (rc != PTY_OK) return rc;
+    DeviceGuard dg(plan->device);
     if (!loss) return fail(plan, PTY_ERR_INVALID_ARG, "loss is null");
     return run_forward(plan, object, probe, positions, tilt, meas_amp, B, loss, loss_per_pos, intensity,
                        static_cast<cudaStream_t>(stream));
@@ -776,11 +725,14 @@ int pty_backward(pty_plan* plan, const void* object, const void* probe, const fl
                  float* g_dz, int32_t flags, void* stream) {
     int rc = check_batch(plan, object, probe, positions, tilt, meas_amp, B);
     if (rc != PTY_OK) return rc;
+    DeviceGuard dg(plan->device);
     if (!g_object) return fail(plan, PTY_ERR_INVALID_ARG, "g_object is null");
     if (g_dz && plan->d.Nz > 1 && !save_hat_of(plan->d))
         return fail(plan, PTY_ERR_INVALID_ARG, "g_dz needs tilt_mode != 0 or PTY_FLAG_SPECTRA");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const bool reuse = !(flags & PTY_BWD_RECOMPUTE) && plan->fwd_valid && plan->f_object == object &&
+    // The saved waves are reused only when the caller says so (PTY_BWD_REUSE_FORWARD: "nothing changed since my
+    // pty_forward_loss") AND the plan has seen no other call since that forward with these very pointers.
+    const bool reuse = (flags & PTY_BWD_REUSE_FORWARD) && plan->fwd_valid && plan->f_object == object &&
                        plan->f_probe == probe && plan->f_positions == positions && plan->f_tilt == tilt &&
                        plan->f_meas == meas_amp && plan->f_B == B && plan->last_stream == st;
     if (!reuse) {
@@ -794,7 +746,9 @@ int pty_backward(pty_plan* plan, const void* object, const void* probe, const fl
 int pty_adam_update(pty_plan* plan, float* theta, const float* grad, float* m, float* v, size_t n, float lr,
                     float beta1, float beta2, float eps, int32_t t, void* stream) {
     if (!plan) return PTY_ERR_INVALID_ARG;
+    DeviceGuard dg(plan->device);
     plan->last_stream = static_cast<cudaStream_t>(stream);
+    plan->fwd_valid = false;            // theta may be one of the arrays the last forward read
     return adam_launch(plan, theta, grad, m, v, n, lr, beta1, beta2, eps, t, static_cast<cudaStream_t>(stream));
 }
 
@@ -802,6 +756,7 @@ int pty_step(pty_plan* plan, void* object, void* probe, float* positions, float*
              int32_t B, const pty_adam* hp, const pty_adam_state* s, double* loss, void* stream) {
     int rc = check_batch(plan, object, probe, positions, tilt, meas_amp, B);
     if (rc != PTY_OK) return rc;
+    DeviceGuard dg(plan->device);
     if (!hp || !s || !loss) return fail(plan, PTY_ERR_INVALID_ARG, "hp, st or loss is null");
     if (!(plan->d.flags & PTY_FLAG_STEP)) return fail(plan, PTY_ERR_INVALID_ARG, "plan was created without PTY_FLAG_STEP");
     const pty_dims& d = plan->d;
@@ -835,6 +790,7 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, con
                   void* h_g_probe, float* h_g_positions, float* h_g_tilt, void* stream) {
     int rc = check_batch(plan, h_object, h_probe, h_positions, h_tilt, h_meas_amp, B);
     if (rc != PTY_OK) return rc;
+    DeviceGuard dg(plan->device);
     if (!(plan->d.flags & PTY_FLAG_HOST)) return fail(plan, PTY_ERR_INVALID_ARG, "plan was created without PTY_FLAG_HOST");
     const pty_dims& d = plan->d;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -870,6 +826,7 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, con
 
 int pty_status(pty_plan* plan, int32_t* device_flags) {
     if (!plan) return PTY_ERR_INVALID_ARG;
+    DeviceGuard dg(plan->device);
     PTY_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
     int flags = 0;
     PTY_CUDA(plan, cudaMemcpy(&flags, plan->d_flags(), sizeof(int), cudaMemcpyDeviceToHost));

@@ -159,8 +159,9 @@ def truth(cfg):
 
 
 def eval_point(cfg, which="A"):
-    """Evaluation point A (perturbed: parity + timing) or B (the paper's default start,
-    PAPER.md:102-104: unit amplitude, phase U[0,1e-8], un-jittered raster; parity only)."""
+    """Evaluation point A (perturbed: parity + timing), B (the paper's default start,
+    PAPER.md:102-104: unit amplitude, phase U[0,1e-8], un-jittered raster; parity only) or
+    Bp (B with phase U[0,1e-2]: a near-vacuum start whose dark field is above float32 noise)."""
     if which == "A":
         rng = np.random.default_rng(1000 * cfg.c + 4)
         pert = np.clip(rng.normal(0.0, 0.2, (cfg.n_positions, 2)), -0.6, 0.6)
@@ -170,6 +171,14 @@ def eval_point(cfg, which="A"):
     if which == "B":
         rng = np.random.default_rng(1000 * cfg.c + 1)
         phase = rng.uniform(0.0, 1e-8, (cfg.Nz, cfg.H, cfg.W))
+        return {"object": np.exp(1j * phase).astype(np.complex64), "probe": make_probe(cfg, 0.3),
+                "positions": raster(cfg).astype(np.float32),
+                "tilt": np.zeros(2, dtype=np.float32)}
+    if which == "Bp":
+        # B': the same start with the phase range raised to U[0, 1e-2] -- still "unit amplitude, small random
+        # phase", but the dark field it scatters sits well above float32 rounding noise (R26)
+        rng = np.random.default_rng(1000 * cfg.c + 1)
+        phase = rng.uniform(0.0, 1e-2, (cfg.Nz, cfg.H, cfg.W))
         return {"object": np.exp(1j * phase).astype(np.complex64), "probe": make_probe(cfg, 0.3),
                 "positions": raster(cfg).astype(np.float32),
                 "tilt": np.zeros(2, dtype=np.float32)}
