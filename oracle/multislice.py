@@ -16,7 +16,7 @@ Conventions (readings R1, R2, R4, R5, R8, R15):
 
 All inputs are upcast to float64/complex128 on entry, so the float32 arrays the GPU
 receives are seen bit-identically here.  ``numpy.fft`` is the one library primitive used
-as a step; it is pinned against a brute-force O(N^4) DFT in tests/test_oracle_dft.py.
+as a step; it is pinned against a brute-force O(N^4) DFT in tests/test_oracle_pins.py.
 """
 from __future__ import annotations
 
@@ -29,7 +29,7 @@ __all__ = [
     "Geometry", "dft2", "idft2", "split_position", "shift_kernel", "shift_probe",
     "shift_probe_adjoint", "crop", "crop_adjoint_add", "propagator_phase", "propagator",
     "propagate", "propagate_adjoint", "forward_position", "intensity_batch",
-    "loss_from_intensity", "forward_loss_batch", "grad_position", "grad_batch",
+    "loss_from_intensity", "forward_loss_batch", "backprop_position", "grad_position", "grad_batch",
     "loss_gaussian_eq5", "adam_step",
 ]
 
@@ -198,25 +198,19 @@ def forward_loss_batch(obj, probe, positions, tilt, meas_amp, geom):
 
 
 # --------------------------------------------------------------------------- B1-B8
-def grad_position(obj, probe, p, tilt, a, geom, g_obj, g_probe):
-    """B1-B8 for one position.  Adds into ``g_obj`` [Nz,H,W] and ``g_probe`` [M,N,N]
-    (complex128) and returns (loss_b, g_pos [2], g_tilt [2], g_dz).
+def backprop_position(f, probe, dLdI, tilt, geom, g_obj, g_probe):
+    """B2-B8 for one position, for ANY loss that depends on the model through I_b(k) only:
+    ``dLdI`` [N,N] = dL/dI_b(k), so that g_Psi^(m) = 2 dLdI Psi^(m) (I = sum_m |Psi|^2, convention R15).
 
-    Hand-derived adjoint of F1-F8 (the paper uses reverse-mode AD, PAPER.md:110; the
-    formulas are SURVEY.md §8(c) B1-B8, convention R15, position gradient R3).
+    ``f`` is the dict of :func:`forward_position`.  Adds into ``g_obj`` [Nz,H,W] and ``g_probe`` [M,N,N]
+    (complex128) and returns (g_pos [2], g_tilt [2], g_dz).  Used with dLdI = 1 - a/sqrt(I) for the amplitude
+    loss (B1) and with the weighted total of Eq. 5-9 (oracle/losses.py).
     """
-    f = forward_position(obj, probe, p, tilt, geom)
     probe = np.asarray(probe, dtype=np.complex128)
-    a = np.asarray(a, dtype=np.float64)
     Nz = len(f["psi"])
     N = probe.shape[-1]
-    I, Psi, O, Mk = f["I"], f["Psi"], f["O"], f["M"]
-    sqrtI = np.sqrt(I)
-    loss_b = float(np.sum((sqrtI - a) ** 2))                           # F8
-    w = np.zeros_like(I)                                               # B1 (R14)
-    nz = I > 0
-    w[nz] = 1.0 - a[nz] / sqrtI[nz]
-    g = idft2(2.0 * w[None] * Psi)                                     # B2: g wrt phi_Nz
+    Psi, O, Mk = f["Psi"], f["O"], f["M"]
+    g = idft2(2.0 * np.asarray(dLdI, dtype=np.float64)[None] * Psi)    # B2: g wrt phi_Nz
     D = np.zeros((N, N))
     for s in range(Nz - 1, -1, -1):
         crop_adjoint_add(g_obj[s], f["r"],                             # B3
@@ -239,6 +233,25 @@ def grad_position(obj, probe, p, tilt, a, geom, g_obj, g_probe):
                                                np.sum(D * kx) / math.cos(tx) ** 2])
     g_dz = float(np.sum(D * (-np.pi * geom.lam * (kx * kx + ky * ky)
                              + 2.0 * np.pi * (kx * math.tan(tx) + ky * math.tan(ty)))))
+    return g_pos, g_tilt, g_dz
+
+
+def grad_position(obj, probe, p, tilt, a, geom, g_obj, g_probe):
+    """B1-B8 for one position.  Adds into ``g_obj`` [Nz,H,W] and ``g_probe`` [M,N,N]
+    (complex128) and returns (loss_b, g_pos [2], g_tilt [2], g_dz).
+
+    Hand-derived adjoint of F1-F8 (the paper uses reverse-mode AD, PAPER.md:110; the
+    formulas are SURVEY.md §8(c) B1-B8, convention R15, position gradient R3).
+    """
+    f = forward_position(obj, probe, p, tilt, geom)
+    a = np.asarray(a, dtype=np.float64)
+    I = f["I"]
+    sqrtI = np.sqrt(I)
+    loss_b = float(np.sum((sqrtI - a) ** 2))                           # F8
+    w = np.zeros_like(I)                                               # B1 (R14): dL/dI = 1 - a/sqrt(I)
+    nz = I > 0
+    w[nz] = 1.0 - a[nz] / sqrtI[nz]
+    g_pos, g_tilt, g_dz = backprop_position(f, probe, w, tilt, geom, g_obj, g_probe)
     return loss_b, g_pos, g_tilt, g_dz
 
 

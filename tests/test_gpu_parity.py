@@ -315,6 +315,35 @@ def test_run_to_run_repeatability_bound(pty):
     assert a["loss"][0] == pytest.approx(b["loss"][0], rel=1e-6)
 
 
+def test_bitwise_repeatability_when_no_output_is_shared(pty):
+    """Race check without compute-sanitizer (closed on this pool, profiles/r02_sanitizer.md): with ONE probe mode and
+    64 non-overlapping patches every output element except g_probe receives exactly one contribution, so the
+    intensities, per-position losses, object and position gradients must be BIT-identical from run to run whatever
+    the timing of the named-barrier hand-over of the transpose buffer, the TMEM slots and the atomics' order.
+    Twelve runs, the later ones with a second stream keeping other CTAs on the SMs to perturb the timing."""
+    cfg = synth.get_config(4, M=1, Nz=3)
+    g = 128 * np.arange(8, dtype=np.float32) + 32.0
+    yy, xx = np.meshgrid(g, g, indexing="ij")
+    rng = np.random.default_rng(21)
+    pos = (np.stack([yy.ravel(), xx.ravel()], 1) + rng.uniform(-0.4, 0.4, (64, 2))).astype(np.float32)
+    ev = synth.eval_point(cfg, "A")
+    meas = np.sqrt(rng.poisson(3.0, (64, cfg.N, cfg.N))).astype(np.float32)
+    case = {"cfg": cfg, "object": ev["object"], "probe": np.ascontiguousarray(ev["probe"][:1]), "positions": pos,
+            "tilt": None, "tilt_mode": 0, "meas": meas}
+    first = run_gpu(pty, case)
+    side = torch.cuda.Stream()
+    junk = torch.randn(4096, 4096, device="cuda")
+    for rep_ in range(11):
+        if rep_ >= 4:
+            with torch.cuda.stream(side):
+                for _ in range(3):
+                    junk = junk @ junk * 1e-3
+        r = run_gpu(pty, case, plan=first["plan"])
+        for k in ("intensity", "loss_per_pos", "g_object", "g_positions"):
+            assert np.array_equal(first[k], r[k]), (k, rep_)
+    torch.cuda.synchronize()
+
+
 def test_grad_host_end_to_end(pty):
     cfg = synth.get_config(1)
     case = make_case(1, "A", synth.minibatch(cfg, 1, cfg.B))
@@ -476,7 +505,9 @@ def test_pty_step_with_global_tilt_on_multislice(pty):
     np.testing.assert_allclose(tilt.cpu().numpy(), new_tilt, rtol=1e-3, atol=1e-9)
     np.testing.assert_allclose(state["m_tilt"].cpu().numpy(), m_t, rtol=2e-3)
     new_pos, _, _ = oracle.adam_step(pos0, ref["g_positions"], np.zeros((B, 2)), np.zeros((B, 2)), 1, 1e-3)
-    assert rel_l2(pos.cpu().numpy() - pos0, new_pos - pos0) <= 1e-3
+    # positions ~ 2e2 px in float32 (ulp 1.5e-5): the 1e-3 px step is resolved to about 1 %
+    np.testing.assert_allclose(pos.cpu().numpy(), new_pos, rtol=0, atol=3.1e-5)
+    assert np.all(np.sign(pos.cpu().numpy() - pos0) == np.sign(new_pos - pos0))
     new_probe, _, _ = oracle.adam_step(ev["probe"], ref["g_probe"], np.zeros(ev["probe"].size * 2),
                                        np.zeros(ev["probe"].size * 2), 1, 1e-4)
     gp = ref["g_probe"].view(np.float64)
