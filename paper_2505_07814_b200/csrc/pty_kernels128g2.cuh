@@ -22,6 +22,10 @@
 #include "pty_fft128.cuh"
 #include "pty_kernels.cuh"
 
+#ifndef PTY_G2_D
+#define PTY_G2_D 3      // chunks of saved-wave / object rows in flight in the adjoint's streaming step
+#endif
+
 namespace pty {
 
 struct G2Smem {
@@ -212,8 +216,10 @@ PTY_DEV void g2_accumulate(const G2& c, int slot, float v) {
 
 // ------------------------------------------------------------------------------ forward (a2-a5)
 // item = b M + m; live = false for the padding item of an odd grid (same control flow, no global writes).
-PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
-    constexpr int N = 128, NT = F128::NT, P = F128::P;
+// HAT: keep the propagated spectra (tilt / dz gradients); a compile-time switch so that the common no-tilt kernels
+// carry neither the code nor the registers of that path.
+template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
+    constexpr int N = 128, NT = F128::NT;
     const int b = item / A.M, m = item % A.M;
     int ry, rx;
     setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
@@ -273,11 +279,11 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
             const int o = 2 * c.gg + h;
             g2_ld_slots(c, o, v);
             g2_radix4<-1>(c, o, v);
-            float2* hat = A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + s) * NN + 128 * o + c.c : nullptr;
+            float2* hat = HAT ? A.ws_hat + (bm * (A.Nz - 1) + s) * NN + 128 * o + c.c : nullptr;
 #pragma unroll
             for (int r = 0; r < 32; ++r) {
                 v[r] = cmul(v[r], cmul(my, c.Mx[c.kx(o, r)]));
-                if (hat && live) st_stream2(hat + r * NT, v[r]);
+                if (HAT && live) st_stream2(hat + r * NT, v[r]);
             }
             g2_radix4<+1>(c, o, v);
             g2_st_slots(c, o, v);
@@ -308,7 +314,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
 }
 
 // ------------------------------------------------------------------------------ adjoint (a7-a13)
-PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
+template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
     constexpr int N = 128, NT = F128::NT;
     const int b = item / A.M, m = item % A.M;
     int ry, rx;
@@ -349,7 +355,7 @@ PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
         }
         tmem_wait_st();
         {
-            constexpr int D = 5;
+            constexpr int D = PTY_G2_D;
             const size_t ostride = (size_t)4 * A.W;
             const float2* obj0 = A.object + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
             float2* gobj0 = A.g_object + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
@@ -381,7 +387,10 @@ PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
                 tmem_st4(tb0 + 64u * ((J) >> 3) + 8u * ((J) & 7), gb[(J) & 1]);                           \
                 if ((J) + D < 16) PTY_G2_ISSUE((J) + D)                                                   \
             }
-            PTY_G2_ISSUE(0) PTY_G2_ISSUE(1) PTY_G2_ISSUE(2) PTY_G2_ISSUE(3) PTY_G2_ISSUE(4)
+            PTY_G2_ISSUE(0) PTY_G2_ISSUE(1) PTY_G2_ISSUE(2)
+            if (D > 3) PTY_G2_ISSUE(3)
+            if (D > 4) PTY_G2_ISSUE(4)
+            if (D > 5) PTY_G2_ISSUE(5)
             tmem_ld4(tb0, gb[0]);
             PTY_G2_STEP(0) PTY_G2_STEP(1) PTY_G2_STEP(2) PTY_G2_STEP(3) PTY_G2_STEP(4) PTY_G2_STEP(5)
             PTY_G2_STEP(6) PTY_G2_STEP(7) PTY_G2_STEP(8) PTY_G2_STEP(9) PTY_G2_STEP(10) PTY_G2_STEP(11)
@@ -407,7 +416,7 @@ PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
             const int o = 2 * c.gg + h;
             g2_ld_slots(c, o, v);
             g2_radix4<-1>(c, o, v);
-            if (A.save_hat) {
+            if (HAT) {
                 const float2* hat = A.ws_hat + (bm * (A.Nz - 1) + (s - 1)) * NN + 128 * o + c.c;
 #pragma unroll
                 for (int r = 0; r < 32; ++r) {
@@ -453,7 +462,7 @@ PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
     }
     g2_accumulate(c, 0, accy);
     g2_accumulate(c, 1, accx);
-    if (A.save_hat) {
+    if (HAT) {
         g2_accumulate(c, 2, acc_ky);
         g2_accumulate(c, 3, acc_kx);
         g2_accumulate(c, 4, acc_k2);
@@ -465,7 +474,7 @@ PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
             red_add(A.g_pos + 2 * b, two_pi * c.red[0]);
             red_add(A.g_pos + 2 * b + 1, two_pi * c.red[1]);
         }
-        if (A.save_hat) {
+        if (HAT) {
             red_add(A.dsum + 4 * b, c.red[2]);
             red_add(A.dsum + 4 * b + 1, c.red[3]);
             red_add(A.dsum + 4 * b + 2, c.red[4]);

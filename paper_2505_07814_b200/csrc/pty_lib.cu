@@ -83,18 +83,29 @@ __device__ __forceinline__ void release_cta128(unsigned char* smem) {
 }
 
 // N = 128, two items per CTA (pty_kernels128g2.cuh): group G of CTA x owns item 2 x + G
-__global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A) {
+template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const G2 c = make_g2(smem);
-    const int n = A.B * A.M, item = 2 * blockIdx.x + c.G;
-    fwd_body_g2(A, c, min(item, n - 1), item < n);
+    // persistent CTAs: TMEM allocation and the twiddle table once per SM; CTA x takes the item pairs x, x + grid, ...
+    // (both groups run the same number of bodies: the hand-over of the transpose buffer is balanced per body)
+    const int n = A.B * A.M;
+    for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
+        const int item = it + c.G;
+        fwd_body_g2<HAT>(A, c, min(item, n - 1), item < n);
+        c.grp_sync();            // the next body rewrites the group's tables and reduction slots
+    }
     release_g2(smem);
 }
-__global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_kernel(const KArgs A) {
+template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_kernel(const KArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const G2 c = make_g2(smem);
-    const int n = A.B * A.M, item = 2 * blockIdx.x + c.G;
-    bwd_body_g2(A, c, min(item, n - 1), item < n);
+    const int n = A.B * A.M;
+    for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
+        int item = it + c.G;
+        asm volatile("" : "+r"(item));           // keep per-item address arithmetic inside the body (register pressure)
+        bwd_body_g2<HAT>(A, c, min(item, n - 1), item < n);
+        c.grp_sync();
+    }
     release_g2(smem);
 }
 
@@ -465,14 +476,22 @@ template <class SH> cudaError_t launch_fwd_sh(pty_plan* p, const KArgs& A, cudaS
 template <class SH> cudaError_t launch_bwd_sh(pty_plan* p, const KArgs& A, cudaStream_t st) {
     return launch(p, pty_bwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
+int g2_grid(const pty_plan* p, const KArgs& A) {      // one persistent CTA per SM, or fewer when there is less work
+    const int pairs = (A.B * A.M + 1) / 2;
+    return pairs < p->num_sms ? pairs : p->num_sms;
+}
 cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 0, st);
-    if (p->d.N == 128) return launch(p, pty_fwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
+    if (p->d.N == 128)
+        return A.save_hat ? launch(p, pty_fwd128g2_kernel<true>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A)
+                          : launch(p, pty_fwd128g2_kernel<false>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A);
     return p->d.N == 64 ? launch_fwd_sh<Shape<64>>(p, A, st) : launch_fwd_sh<Shape<256>>(p, A, st);
 }
 cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 1, st);
-    if (p->d.N == 128) return launch(p, pty_bwd128g2_kernel, (A.B * A.M + 1) / 2, F128::NT, G2Smem::bytes, 1, st, A);
+    if (p->d.N == 128)
+        return A.save_hat ? launch(p, pty_bwd128g2_kernel<true>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A)
+                          : launch(p, pty_bwd128g2_kernel<false>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A);
     return p->d.N == 64 ? launch_bwd_sh<Shape<64>>(p, A, st) : launch_bwd_sh<Shape<256>>(p, A, st);
 }
 // plain 2-D FFT of `items` planes (N = 64, 256): P^ = F[P] / N and g_probe = F^-1[G^_P] / N
@@ -653,9 +672,13 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
     if (e == cudaSuccess && dims->N == 64) e = set_smem_attrs<Shape<64>>();
     if (e == cudaSuccess && dims->N == 256) e = set_smem_attrs<Shape<256>>();
     if (e == cudaSuccess && dims->N == 128) {
-        e = cudaFuncSetAttribute(pty_fwd128g2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+        e = cudaFuncSetAttribute(pty_fwd128g2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(pty_bwd128g2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+            e = cudaFuncSetAttribute(pty_fwd128g2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_probe_hat128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
         if (e == cudaSuccess)
