@@ -35,7 +35,10 @@
  * past a call (except the workspace given to pty_create).
  *
  * Execution.  Everything is enqueued on the given stream; no call synchronises except
- * pty_status and the *_host entry points.  One plan per stream; a plan is not thread-safe.
+ * pty_status, pty_loss_terms, pty_profile_read and the *_host entry points.  The enqueue-only
+ * calls make no allocation and no synchronisation, so a sequence of them on fixed pointers can
+ * be recorded once with CUDA stream capture and replayed as a graph (launch-bound small
+ * configurations; tests/test_gpu_features.py).  One plan per stream; a plan is not thread-safe.
  *
  * Errors.  Every function returns PTY_OK (0) or a negative PTY_ERR_* code; the text of the last
  * error of a plan is available from pty_last_error.  No C++ exception crosses this boundary.
@@ -65,6 +68,8 @@ extern "C" {
                                        when tilt_mode == 0 (implied by tilt_mode != 0)        */
 #define PTY_FLAG_STEP          2    /* reserve gradient buffers in the workspace: pty_step     */
 #define PTY_FLAG_HOST          4    /* reserve device staging buffers: pty_grad_host           */
+#define PTY_FLAG_AMP_PHASE     8    /* reserve the composed object, its gradient and the patch
+                                       coverage map: pty_*_ap (amplitude / phase object)       */
 
 /* pty_backward flags */
 #define PTY_BWD_ACCUMULATE     1    /* add into the gradient outputs instead of overwriting    */
@@ -84,7 +89,44 @@ typedef struct pty_dims {
     int32_t tilt_mode;    /* 0: no tilt (tilt pointers ignored); 1: one global tilt [2];
                              2: one tilt per position [B][2]                                  */
     int32_t flags;        /* PTY_FLAG_*                                                       */
+    int32_t n_obj;        /* mixed object states N (Eq. 2): object and g_object are
+                             [n_obj][Nz][H][W], I = sum_m sum_n |F psi^(m)(n)|^2; 0 or 1 = one state    */
 } pty_dims;
+
+/* The paper's loss family (R27-R30).  mode 0 (default): the plain amplitude sum
+ *   L = sum_b sum_k (sqrt(I) - a)^2 of the north_star.  mode 1: Eq. 9,
+ *   L_total = w_gaussian L_Gaussian(Eq. 5, p = 1/2) + w_poisson L_Poisson(Eq. 6, p = 1, eps) + w_pacbed L_PACBED
+ *   (Eq. 7, p = 1/2) + w_sparse L_sparse(Eq. 8, p = 1; only the amplitude / phase entry points know the phase),
+ *   every average taken over the detector and the minibatch of the call.  In both modes loss_per_pos[b] is the
+ *   plain sum of position b, and every gradient is that of the scalar written to `loss`. */
+typedef struct pty_loss {
+    int32_t mode;
+    float w_gaussian, w_poisson, w_pacbed, w_sparse;
+    float eps;            /* Poisson epsilon, 1e-6 in the paper                         */
+} pty_loss;
+
+/* Adam for the amplitude / phase parameterisation (separate learning rates). */
+typedef struct pty_adam_ap {
+    float lr_amp, lr_phase, lr_probe, lr_positions, lr_tilt;
+    float beta1, beta2, eps;
+    int32_t t;
+} pty_adam_ap;
+typedef struct pty_adam_state_ap {
+    float *m_amp, *v_amp, *m_phase, *v_phase;        /* [n_obj*Nz*H*W] each */
+    float *m_probe, *v_probe, *m_positions, *v_positions, *m_tilt, *v_tilt;
+} pty_adam_state_ap;
+
+/* Per-iteration constraints of the paper's reconstructions (R31). */
+typedef struct pty_constraints {
+    int32_t ortho_probe;      /* 1: replace the probe modes by the orthogonal modes of the same mixed state,
+                                 ordered by decreasing power (Thibault & Menzel 2013)                  */
+    float   sigma_z;          /* > 0: r_z filter, Eq. 13 -- Gaussian blur along depth (in slices) of amp and
+                                 phase; taps exp(-j^2 / 2 sigma_z^2), |j| <= max(1, ceil(2 sigma_z)) <= 8,
+                                 normalised, end slices replicated                                     */
+    int32_t phase_positive;   /* 1: phase = max(phase, 0)                                               */
+    int32_t clamp_amp;        /* 1: amp = min(max(amp, amp_min), amp_max)                               */
+    float   amp_min, amp_max;
+} pty_constraints;
 
 /* Adam hyper-parameters (Kingma & Ba with bias correction; R20).
  * A learning rate of 0 freezes that parameter group (its moments are left untouched). */
@@ -140,6 +182,37 @@ int pty_backward(pty_plan* plan, const void* object, const void* probe,
                  const float* positions, const float* tilt, const float* meas_amp, int32_t B,
                  void* g_object, void* g_probe, float* g_positions, float* g_tilt, float* g_dz,
                  int32_t flags, void* stream);
+
+/* Select the loss of every later call on this plan (NULL = mode 0).  Host struct, copied. */
+int pty_set_loss(pty_plan* plan, const pty_loss* cfg);
+
+/* The four terms (L_Gaussian, L_Poisson, L_PACBED, L_sparse) of the last mode-1 forward on this plan, to host;
+ * synchronises the plan's stream.  L_PACBED and L_sparse are evaluated only when they carry a non-zero weight
+ * (0 otherwise). */
+int pty_loss_terms(pty_plan* plan, double* terms4);
+
+/* Amplitude / phase object: O = amp exp(i phase), both [n_obj][Nz][H][W] f32.  The complex object is
+ * composed into the workspace (plan needs PTY_FLAG_AMP_PHASE) and the calls below behave like their complex
+ * counterparts; g_amp = Re(conj(g_O) e^{i phase}), g_phase = Im(g_O conj(O)) + w_sparse dL_sparse/dphase.  With loss
+ * mode 1 the sparsity term Eq. 8 (mean |phase| over the patches of the minibatch) is part of `loss`. */
+int pty_forward_loss_ap(pty_plan* plan, const float* amp, const float* phase, const void* probe,
+                        const float* positions, const float* tilt, const float* meas_amp, int32_t B,
+                        double* loss, float* loss_per_pos, float* intensity, void* stream);
+int pty_backward_ap(pty_plan* plan, const float* amp, const float* phase, const void* probe,
+                    const float* positions, const float* tilt, const float* meas_amp, int32_t B,
+                    float* g_amp, float* g_phase, void* g_probe, float* g_positions, float* g_tilt, float* g_dz,
+                    int32_t flags, void* stream);
+/* The paper's minibatch update: forward, Eq. 9 loss, gradients, Adam on amplitude, phase, probe, positions, tilt
+ * (plan needs PTY_FLAG_STEP | PTY_FLAG_AMP_PHASE). */
+int pty_step_ap(pty_plan* plan, float* amp, float* phase, void* probe, float* positions, float* tilt,
+                const float* meas_amp, int32_t B, const pty_adam_ap* hp, const pty_adam_state_ap* st,
+                double* loss, void* stream);
+
+/* Apply the constraints in place: amp / phase [n_obj][Nz][H][W] f32 (either may be NULL), probe [M][N][N] c64
+ * (may be NULL when ortho_probe == 0; M <= 32 for the orthogonalisation).  Enqueue-only. */
+int pty_constrain(pty_plan* plan, float* amp, float* phase, void* probe, const pty_constraints* c, void* stream);
+/* Eq. 13 as printed, on a complex object [n_obj][Nz][H][W] c64 in place (real kernel: re and im are blurred). */
+int pty_rz_filter_object(pty_plan* plan, void* object, float sigma_z, void* stream);
 
 /* One optimisation step: forward, loss, gradient and an Adam update of object, probe, positions
  * and tilt in place (plan needs PTY_FLAG_STEP).  loss [1] f64 device = L before

@@ -23,18 +23,40 @@ lib = C.CDLL(LIB_PATH)
 
 PTY_OK, PTY_ERR_INVALID_ARG, PTY_ERR_UNSUPPORTED = 0, -1, -2
 PTY_ERR_WORKSPACE, PTY_ERR_CUDA, PTY_ERR_BOUNDS = -3, -4, -5
-PTY_FLAG_SPECTRA, PTY_FLAG_STEP, PTY_FLAG_HOST = 1, 2, 4
+PTY_FLAG_SPECTRA, PTY_FLAG_STEP, PTY_FLAG_HOST, PTY_FLAG_AMP_PHASE = 1, 2, 4, 8
 PTY_BWD_ACCUMULATE, PTY_BWD_REUSE_FORWARD = 1, 4
 
 EXPORTS = ["pty_workspace_bytes", "pty_create", "pty_destroy", "pty_forward_loss", "pty_backward",
            "pty_step", "pty_adam_update", "pty_grad_host", "pty_status", "pty_profile",
-           "pty_profile_read", "pty_launch_count", "pty_last_error", "pty_version"]
+           "pty_profile_read", "pty_set_loss", "pty_loss_terms", "pty_forward_loss_ap", "pty_backward_ap",
+           "pty_step_ap", "pty_constrain", "pty_rz_filter_object", "pty_launch_count", "pty_last_error", "pty_version"]
+_INT_RETURNS = EXPORTS[:18]
 
 
 class pty_dims(C.Structure):
     _fields_ = [("Nz", C.c_int32), ("H", C.c_int32), ("W", C.c_int32), ("M", C.c_int32), ("N", C.c_int32),
                 ("Bmax", C.c_int32), ("dz", C.c_float), ("lam", C.c_float), ("dx", C.c_float),
-                ("tilt_mode", C.c_int32), ("flags", C.c_int32)]
+                ("tilt_mode", C.c_int32), ("flags", C.c_int32), ("n_obj", C.c_int32)]
+
+
+class pty_loss(C.Structure):
+    _fields_ = [("mode", C.c_int32), ("w_gaussian", C.c_float), ("w_poisson", C.c_float), ("w_pacbed", C.c_float),
+                ("w_sparse", C.c_float), ("eps", C.c_float)]
+
+
+class pty_adam_ap(C.Structure):
+    _fields_ = [("lr_amp", C.c_float), ("lr_phase", C.c_float), ("lr_probe", C.c_float), ("lr_positions", C.c_float),
+                ("lr_tilt", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("t", C.c_int32)]
+
+
+class pty_adam_state_ap(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("m_amp", "v_amp", "m_phase", "v_phase", "m_probe", "v_probe", "m_positions",
+                                          "v_positions", "m_tilt", "v_tilt")]
+
+
+class pty_constraints(C.Structure):
+    _fields_ = [("ortho_probe", C.c_int32), ("sigma_z", C.c_float), ("phase_positive", C.c_int32),
+                ("clamp_amp", C.c_int32), ("amp_min", C.c_float), ("amp_max", C.c_float)]
 
 
 class pty_adam(C.Structure):
@@ -68,7 +90,15 @@ lib.pty_launch_count.restype = C.c_int64
 lib.pty_last_error.argtypes = [_vp]
 lib.pty_last_error.restype = C.c_char_p
 lib.pty_version.restype = C.c_char_p
-for _n in EXPORTS[:11]:
+lib.pty_set_loss.argtypes = [_vp, C.POINTER(pty_loss)]
+lib.pty_loss_terms.argtypes = [_vp, C.POINTER(C.c_double)]
+lib.pty_forward_loss_ap.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, _vp, _vp, _vp, _vp]
+lib.pty_backward_ap.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, _vp]
+lib.pty_step_ap.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.POINTER(pty_adam_ap),
+                            C.POINTER(pty_adam_state_ap), _vp, _vp]
+lib.pty_constrain.argtypes = [_vp, _vp, _vp, _vp, C.POINTER(pty_constraints), _vp]
+lib.pty_rz_filter_object.argtypes = [_vp, _vp, C.c_float, _vp]
+for _n in _INT_RETURNS:
     getattr(lib, _n).restype = C.c_int
 
 
@@ -98,10 +128,10 @@ def _stream():
 class Plan:
     """Owns a pty_plan and its workspace (a torch uint8 CUDA tensor)."""
 
-    def __init__(self, Nz, H, W, M, N, Bmax, dz, lam, dx, tilt_mode=0, flags=0, device=0):
+    def __init__(self, Nz, H, W, M, N, Bmax, dz, lam, dx, tilt_mode=0, flags=0, device=0, n_obj=1):
         if not torch.cuda.is_available():
             raise RuntimeError("pty needs a CUDA device (sm_100a); there is no CPU fallback")
-        self.dims = pty_dims(Nz, H, W, M, N, Bmax, dz, lam, dx, tilt_mode, flags)
+        self.dims = pty_dims(Nz, H, W, M, N, Bmax, dz, lam, dx, tilt_mode, flags, n_obj)
         nbytes = C.c_size_t(0)
         rc = lib.pty_workspace_bytes(C.byref(self.dims), C.byref(nbytes))
         if rc != PTY_OK:
@@ -160,6 +190,57 @@ class Plan:
             _ptr(loss, torch.float64, "cuda"), _stream()))
         return loss
 
+    def set_loss(self, mode=0, w_gaussian=1.0, w_poisson=0.0, w_pacbed=0.0, w_sparse=0.0, eps=1e-6):
+        cfg = pty_loss(mode, w_gaussian, w_poisson, w_pacbed, w_sparse, eps)
+        self._check(lib.pty_set_loss(self._h, C.byref(cfg)))
+
+    def loss_terms(self):
+        """{'gaussian', 'poisson', 'pacbed', 'sparse'} of the last loss-mode-1 forward (synchronises)."""
+        out = (C.c_double * 4)()
+        self._check(lib.pty_loss_terms(self._h, out))
+        return dict(zip(("gaussian", "poisson", "pacbed", "sparse"), list(out)))
+
+    def forward_loss_ap(self, amp, phase, probe, positions, tilt, meas_amp, loss=None, loss_per_pos=None, intensity=None):
+        loss = self._loss if loss is None else loss
+        self._check(lib.pty_forward_loss_ap(
+            self._h, _ptr(amp, torch.float32, "cuda"), _ptr(phase, torch.float32, "cuda"),
+            _ptr(probe, torch.complex64, "cuda"), _ptr(positions, torch.float32, "cuda"),
+            _ptr(tilt, torch.float32, "cuda"), _ptr(meas_amp, torch.float32, "cuda"), positions.shape[0],
+            _ptr(loss, torch.float64, "cuda"), _ptr(loss_per_pos, torch.float32, "cuda"),
+            _ptr(intensity, torch.float32, "cuda"), _stream()))
+        return loss
+
+    def backward_ap(self, amp, phase, probe, positions, tilt, meas_amp, g_amp, g_phase, g_probe=None, g_positions=None,
+                    g_tilt=None, g_dz=None, flags=0):
+        self._check(lib.pty_backward_ap(
+            self._h, _ptr(amp, torch.float32, "cuda"), _ptr(phase, torch.float32, "cuda"),
+            _ptr(probe, torch.complex64, "cuda"), _ptr(positions, torch.float32, "cuda"),
+            _ptr(tilt, torch.float32, "cuda"), _ptr(meas_amp, torch.float32, "cuda"), positions.shape[0],
+            _ptr(g_amp, torch.float32, "cuda"), _ptr(g_phase, torch.float32, "cuda"),
+            _ptr(g_probe, torch.complex64, "cuda"), _ptr(g_positions, torch.float32, "cuda"),
+            _ptr(g_tilt, torch.float32, "cuda"), _ptr(g_dz, torch.float32, "cuda"), flags, _stream()))
+
+    def step_ap(self, amp, phase, probe, positions, tilt, meas_amp, hp: pty_adam_ap, state: dict, loss=None):
+        loss = self._loss if loss is None else loss
+        st = pty_adam_state_ap(*[_ptr(state.get(n), torch.float32, "cuda") for n, _ in pty_adam_state_ap._fields_])
+        self._check(lib.pty_step_ap(
+            self._h, _ptr(amp, torch.float32, "cuda"), _ptr(phase, torch.float32, "cuda"),
+            _ptr(probe, torch.complex64, "cuda"), _ptr(positions, torch.float32, "cuda"),
+            _ptr(tilt, torch.float32, "cuda"), _ptr(meas_amp, torch.float32, "cuda"), positions.shape[0],
+            C.byref(hp), C.byref(st), _ptr(loss, torch.float64, "cuda"), _stream()))
+        return loss
+
+    def constrain(self, amp=None, phase=None, probe=None, ortho_probe=False, sigma_z=0.0, phase_positive=False,
+                  clamp_amp=None):
+        lo, hi = clamp_amp if clamp_amp is not None else (0.0, 0.0)
+        c = pty_constraints(1 if ortho_probe else 0, sigma_z, 1 if phase_positive else 0,
+                            1 if clamp_amp is not None else 0, lo, hi)
+        self._check(lib.pty_constrain(self._h, _ptr(amp, torch.float32, "cuda"), _ptr(phase, torch.float32, "cuda"),
+                                      _ptr(probe, torch.complex64, "cuda"), C.byref(c), _stream()))
+
+    def rz_filter_object(self, obj, sigma_z):
+        self._check(lib.pty_rz_filter_object(self._h, _ptr(obj, torch.complex64, "cuda"), sigma_z, _stream()))
+
     def adam_update(self, theta, grad, m, v, lr, beta1=0.9, beta2=0.999, eps=1e-8, t=1):
         n = theta.numel() * (2 if theta.is_complex() else 1)
         self._check(lib.pty_adam_update(self._h, theta.data_ptr(), grad.data_ptr(), _ptr(m, torch.float32, "cuda"),
@@ -196,7 +277,7 @@ class Plan:
         return lib.pty_last_error(self._h).decode()
 
 
-def plan_for(cfg, Bmax=None, flags=0, device=0):
+def plan_for(cfg, Bmax=None, flags=0, device=0, n_obj=1):
     """Plan for a ``synth.Config``."""
     return Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, cfg.B if Bmax is None else Bmax, cfg.dz, cfg.lam, cfg.dx,
-                tilt_mode=cfg.tilt_mode, flags=flags, device=device)
+                tilt_mode=cfg.tilt_mode, flags=flags, device=device, n_obj=n_obj)

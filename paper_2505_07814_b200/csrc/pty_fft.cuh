@@ -55,6 +55,21 @@ PTY_DEV float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * 
 PTY_DEV float2 cscale(float2 a, float s) { return make_float2(a.x * s, a.y * s); }
 #endif
 PTY_DEV float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
+// variable twiddles of the cross-thread radix-4 stage: packed form behind its own switch (PTY_PK_TW)
+#ifndef PTY_PK_TW
+#define PTY_PK_TW 0
+#endif
+#if PTY_PK_TW
+PTY_DEV float2 cmul_tw(float2 a, float2 w) {      // a * w
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(-w.y, w.y), __fmul2_rn(a, make_float2(w.x, w.x)));
+}
+PTY_DEV float2 cmulc_tw(float2 w, float2 a) {     // conj(w) * a
+    return __ffma2_rn(make_float2(a.y, a.x), make_float2(w.y, -w.y), __fmul2_rn(a, make_float2(w.x, w.x)));
+}
+#else
+PTY_DEV float2 cmul_tw(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
+PTY_DEV float2 cmulc_tw(float2 w, float2 a) { return make_float2(w.x * a.x + w.y * a.y, w.x * a.y - w.y * a.x); }
+#endif
 
 // a * exp(DIR * i * pi/2): forward multiplies by -i, inverse by +i
 template <int DIR> PTY_DEV float2 mul_qi(float2 a) {

@@ -20,10 +20,12 @@ namespace pty {
 
 struct KArgs {
     int Nz, H, W, M, B;
+    int Nobj, MT;         // object states (Eq. 2) and MT = M * Nobj items per position:
+                          // item = b MT + n M + m runs probe mode m through object state n
     int tilt_mode;        // 0 none, 1 global, 2 per position
     int save_hat;         // keep propagated spectra (tilt / dz gradients)
     float dz, lambda, dx;
-    const float2* object;      // [Nz][H][W]
+    const float2* object;      // [Nobj][Nz][H][W]
     const float2* probe_hat;   // [M][N][N]  unitary spectrum of the probe
     const float* positions;    // [B][2]
     const float* tilt;         // [2] or [B][2] or null
@@ -36,11 +38,20 @@ struct KArgs {
     float2* ws_hat;            // [B][M][Nz-1][N][N] spectrum of psi_{s+1} (times 1/N), optional
     float2* GP_hat;            // [M][N][N]   sum_b conj(E_b) F[g_psi0]
     float* dsum;               // [B][4]      sum_k D (k_py, k_px, |k_p|^2)
-    float* seed_w;             // [B][32][512] seed weights 2 (1 - a / sqrt(I)) / N in thread order (N = 128 register path)
+    float* seed_w;             // [B][N][N] seed weights 2 (dL/dI) / N: thread order [r][tid] for N = 128, else natural
     int* flags;                // sticky device flags (bit 0: a crop was clamped)
-    float2* g_object;          // [Nz][H][W]
+    float2* g_object;          // [Nobj][Nz][H][W]
     float* g_pos;              // [B][2]
 };
+
+// item -> position b, probe mode m, offset of object state n in `object` / `g_object`
+PTY_DEV void decode_item(const KArgs& A, int item, int& b, int& m, size_t& obj_off) {
+    b = item / A.MT;
+    const int mm = item - b * A.MT;
+    const int n = mm / A.M;
+    m = mm - n * A.M;
+    obj_off = (size_t)n * A.Nz * A.H * A.W;
+}
 
 template <int N> PTY_DEV float kp_of(int j) { return (float)(j < N / 2 ? j : j - N) * (1.0f / N); }
 
@@ -149,27 +160,23 @@ struct InFwdProp {
     }
 };
 
-// a7 (B1): g_Psi = 2 (1 - a / sqrt(I)) Psi, zero where I = 0; carries the 1/N of the F^-1 (B2)
+// a7 (B1): g_Psi = w Psi with the seed weights w = 2 (dL/dI) / N written by the loss kernels (pty_pointwise.cuh;
+// plain sum: dL/dI = 1 - a / sqrt(I), zero where I = 0); the 1/N is that of the F^-1 (B2)
 struct InSeed {
     const float2* Psi;
-    const float* I;
-    const float* a;
+    const float* Wt;
     template <class SH, int R>
     PTY_DEV void load(const Cta<SH>&, int n2, int, int gline, float2 (&v)[R]) {
         using SI = ShapeInfo<SH>;
-        float iv[R], av[R];
+        float wv[R];
 #pragma unroll
         for (int n1 = 0; n1 < R; ++n1) {
             const int idx = (SI::R2 * n1 + n2) * SI::N + gline;
             v[n1] = ld_stream2(Psi + idx);
-            iv[n1] = ldg1(I + idx);
-            av[n1] = ldg1(a + idx);
+            wv[n1] = ldg1(Wt + idx);
         }
 #pragma unroll
-        for (int n1 = 0; n1 < R; ++n1) {
-            const float w = iv[n1] > 1e-30f ? 2.0f * (1.0f - av[n1] * rsqrt_f(iv[n1])) * (1.0f / SI::N) : 0.f;
-            v[n1] = cscale(v[n1], w);
-        }
+        for (int n1 = 0; n1 < R; ++n1) v[n1] = cscale(v[n1], wv[n1]);
     }
 };
 
@@ -252,11 +259,13 @@ template <class SH>
 PTY_DEV void fwd_body(const KArgs& A, const Cta<SH>& c, int item) {
     using I = ShapeInfo<SH>;
     constexpr int N = SH::N;
-    const int b = item / A.M, m = item % A.M;
+    int b, m;
+    size_t obj_off;
+    decode_item(A, item, b, m, obj_off);
     int ry, rx;
     setup_tables(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
-    const size_t bm = (size_t)b * A.M + m;
+    const size_t bm = (size_t)item;
     InSmem plain;
     {   // psi_0 = F^-1[E . P^]
         InProbe in{A.probe_hat + (size_t)m * NN};
@@ -264,7 +273,7 @@ PTY_DEV void fwd_body(const KArgs& A, const Cta<SH>& c, int item) {
         fft_pass<SH, +1>(c, plain);
     }
     for (int s = 0; s < A.Nz; ++s) {
-        InFwdObj in{A.object + ((size_t)s * A.H + ry) * A.W + rx, A.W, A.ws_psi + (bm * A.Nz + s) * NN};
+        InFwdObj in{A.object + obj_off + ((size_t)s * A.H + ry) * A.W + rx, A.W, A.ws_psi + (bm * A.Nz + s) * NN};
         fft_pass<SH, -1>(c, in);
         fft_pass<SH, -1>(c, plain);
         if (s == A.Nz - 1) break;
@@ -290,20 +299,22 @@ template <class SH>
 PTY_DEV void bwd_body(const KArgs& A, const Cta<SH>& c, int item) {
     using I = ShapeInfo<SH>;
     constexpr int N = SH::N;
-    const int b = item / A.M, m = item % A.M;
+    int b, m;
+    size_t obj_off;
+    decode_item(A, item, b, m, obj_off);
     int ry, rx;
     setup_tables(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
-    const size_t bm = (size_t)b * A.M + m;
+    const size_t bm = (size_t)item;
     InSmem plain;
     {   // B1, B2
-        InSeed in{A.ws_Psi + bm * NN, A.I + (size_t)b * NN, A.meas + (size_t)b * NN};
+        InSeed in{A.ws_Psi + bm * NN, A.seed_w + (size_t)b * NN};
         fft_pass<SH, +1>(c, in);
         fft_pass<SH, +1>(c, plain);
     }
     InBwdProp ip{nullptr, 0.f, 0.f, 0.f};
     for (int s = A.Nz - 1; s >= 0; --s) {
-        const size_t off = ((size_t)s * A.H + ry) * A.W + rx;
+        const size_t off = obj_off + ((size_t)s * A.H + ry) * A.W + rx;
         InBwdObj in{A.object + off, A.W, A.ws_psi + (bm * A.Nz + s) * NN, A.g_object + off};
         fft_pass<SH, -1>(c, in);
         fft_pass<SH, -1>(c, plain);

@@ -98,18 +98,18 @@ template <int DIR> PTY_DEV void g2_radix4(const G2& c, int o, float2 (&v)[32]) {
         const float4 t01 = tw[2 * i], t23 = tw[2 * i + 1];
         if (DIR < 0) {
             float2 a0 = v[i];
-            float2 a1 = cmul(v[8 + i], make_float2(t01.z, t01.w));
-            float2 a2 = cmul(v[16 + i], make_float2(t23.x, t23.y));
-            float2 a3 = cmul(v[24 + i], make_float2(t23.z, t23.w));
+            float2 a1 = cmul_tw(v[8 + i], make_float2(t01.z, t01.w));
+            float2 a2 = cmul_tw(v[16 + i], make_float2(t23.x, t23.y));
+            float2 a3 = cmul_tw(v[24 + i], make_float2(t23.z, t23.w));
             bfly4<-1>(a0, a1, a2, a3);
             v[i] = a0; v[8 + i] = a1; v[16 + i] = a2; v[24 + i] = a3;
         } else {
             float2 a0 = v[i], a1 = v[8 + i], a2 = v[16 + i], a3 = v[24 + i];
             bfly4<+1>(a0, a1, a2, a3);
             v[i] = a0;
-            v[8 + i] = cmulc(make_float2(t01.z, t01.w), a1);
-            v[16 + i] = cmulc(make_float2(t23.x, t23.y), a2);
-            v[24 + i] = cmulc(make_float2(t23.z, t23.w), a3);
+            v[8 + i] = cmulc_tw(make_float2(t01.z, t01.w), a1);
+            v[16 + i] = cmulc_tw(make_float2(t23.x, t23.y), a2);
+            v[24 + i] = cmulc_tw(make_float2(t23.z, t23.w), a3);
         }
     }
 }
@@ -220,12 +220,14 @@ PTY_DEV void g2_accumulate(const G2& c, int slot, float v) {
 // carry neither the code nor the registers of that path.
 template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
     constexpr int N = 128, NT = F128::NT;
-    const int b = item / A.M, m = item % A.M;
+    int b, m;
+    size_t obj_off;
+    decode_item(A, item, b, m, obj_off);
     int ry, rx;
     setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
     c.grp_sync();
     const size_t NN = (size_t)N * N;
-    const size_t bm = (size_t)b * A.M + m;
+    const size_t bm = (size_t)item;
     float2 v[32];
     NoBg bg;
     {   // a2 (K): E . P^ -> inverse x radix-4 -> role blocks
@@ -249,7 +251,7 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
             const int o = 2 * c.gg + h;
-            const float2* obj = A.object + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
+            const float2* obj = A.object + obj_off + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
             const size_t ostride = (size_t)4 * A.W;
             float2 oa[8], ob[8];
 #pragma unroll
@@ -316,12 +318,14 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
 // ------------------------------------------------------------------------------ adjoint (a7-a13)
 template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
     constexpr int N = 128, NT = F128::NT;
-    const int b = item / A.M, m = item % A.M;
+    int b, m;
+    size_t obj_off;
+    decode_item(A, item, b, m, obj_off);
     int ry, rx;
     setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
     c.grp_sync();
     const size_t NN = (size_t)N * N;
-    const size_t bm = (size_t)b * A.M + m;
+    const size_t bm = (size_t)item;
     float2 v[32];
     NoBg bg;
     {   // a7, a8 (K): g_Psi = w Psi, inverse x radix-4 -> role blocks
@@ -357,8 +361,8 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
         {
             constexpr int D = PTY_G2_D;
             const size_t ostride = (size_t)4 * A.W;
-            const float2* obj0 = A.object + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
-            float2* gobj0 = A.g_object + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
+            const float2* obj0 = A.object + obj_off + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
+            float2* gobj0 = A.g_object + obj_off + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
             const float4* psi0 = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 256 * c.gg + c.c;
             const unsigned tb0 = c.blk(2 * c.gg);
             float4 pb[D][2];

@@ -1,5 +1,7 @@
 // pty_lib.cu -- __global__ entry points, the small per-call kernels and the C ABI of include/pty.h.
 // sm_100a only; no cuFFT, no CPU fallback: every step of the hot path runs in the kernels here.
+#include <algorithm>
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -12,6 +14,7 @@
 #include "pty_kernels.cuh"
 #include "pty_kernels128.cuh"
 #include "pty_kernels128g2.cuh"
+#include "pty_pointwise.cuh"
 
 namespace cg = cooperative_groups;
 using namespace pty;
@@ -88,7 +91,7 @@ template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_
     const G2 c = make_g2(smem);
     // persistent CTAs: TMEM allocation and the twiddle table once per SM; CTA x takes the item pairs x, x + grid, ...
     // (both groups run the same number of bodies: the hand-over of the transpose buffer is balanced per body)
-    const int n = A.B * A.M;
+    const int n = A.B * A.MT;
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         const int item = it + c.G;
         fwd_body_g2<HAT>(A, c, min(item, n - 1), item < n);
@@ -99,7 +102,7 @@ template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_
 template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_kernel(const KArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const G2 c = make_g2(smem);
-    const int n = A.B * A.M;
+    const int n = A.B * A.MT;
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         int item = it + c.G;
         asm volatile("" : "+r"(item));           // keep per-item address arithmetic inside the body (register pressure)
@@ -201,35 +204,6 @@ __global__ void pty_prop_table_kernel(int N, float dz, float lambda, float dx, c
     prop_x[j] = make_float2((float)cos(chx), (float)sin(chx));
 }
 
-// a6: L_b = sum_k (sqrt(I_b) - a_b)^2 (Eq. 5, p = 1/2, plain sum); one block per position.
-__global__ void __launch_bounds__(256) pty_loss_kernel(const float* __restrict__ I, const float* __restrict__ a,
-                                                       int NN, double* loss, float* loss_per_pos) {
-    const int b = blockIdx.x;
-    const float4* I4 = reinterpret_cast<const float4*>(I + (size_t)b * NN);
-    const float4* a4 = reinterpret_cast<const float4*>(a + (size_t)b * NN);
-    float acc = 0.f;
-    for (int i = threadIdx.x; i < NN / 4; i += blockDim.x) {
-        const float4 iv = __ldg(I4 + i), av = __ldg(a4 + i);
-        float d;
-        d = sqrtf(iv.x) - av.x; acc += d * d;
-        d = sqrtf(iv.y) - av.y; acc += d * d;
-        d = sqrtf(iv.z) - av.z; acc += d * d;
-        d = sqrtf(iv.w) - av.w; acc += d * d;
-    }
-    __shared__ double part[8];
-    double dacc = (double)acc;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) dacc += __shfl_xor_sync(0xffffffffu, dacc, o);
-    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = dacc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += part[w];
-        if (loss_per_pos) loss_per_pos[b] = (float)t;
-        atomicAdd(loss, t);
-    }
-}
-
 // a13 (B8): tilt and dz gradients from the per-position sums of D(k) (k in cycles/pixel).  One block; thread t
 // handles positions t, t + 256, ...; the sums over b (global tilt, dz) are reduced in double precision.
 __global__ void __launch_bounds__(256) pty_tilt_finalize_kernel(const float* dsum, const float* tilt, int B, int tilt_mode,
@@ -309,6 +283,8 @@ thread_local std::string g_create_error;
 
 struct Layout {
     size_t probe_hat, prop, I, ws_psi, ws_Psi, ws_hat, GP_hat, dsum, seed_w, scalars;
+    size_t stats, Isum, Imsum, taps, gram, eigv, eigl;       // loss family (Eq. 5-9) and constraints
+    size_t ap_object, ap_g_object, ap_cnt;                    // PTY_FLAG_AMP_PHASE
     size_t g_object, g_probe, g_pos, g_tilt;               // PTY_FLAG_STEP / PTY_FLAG_HOST
     size_t h_object, h_probe, h_pos, h_tilt, h_meas;       // PTY_FLAG_HOST staging
     size_t total;
@@ -318,8 +294,11 @@ size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
 
 bool save_hat_of(const pty_dims& d) { return d.Nz > 1 && (d.tilt_mode != 0 || (d.flags & PTY_FLAG_SPECTRA)); }
 
+int n_obj_of(const pty_dims& d) { return d.n_obj > 1 ? d.n_obj : 1; }
+
 int validate_dims(const pty_dims* d, std::string& err) {
     if (!d) { err = "dims is null"; return PTY_ERR_INVALID_ARG; }
+    if (d->n_obj < 0 || d->n_obj > 64) { err = "n_obj must be in [0, 64]"; return PTY_ERR_INVALID_ARG; }
     if (d->Nz < 1 || d->M < 1 || d->Bmax < 1 || d->H < 1 || d->W < 1) { err = "non-positive dimension"; return PTY_ERR_INVALID_ARG; }
     if (d->tilt_mode < 0 || d->tilt_mode > 2) { err = "tilt_mode must be 0, 1 or 2"; return PTY_ERR_INVALID_ARG; }
     if (!(d->dx > 0.f) || !(d->lambda >= 0.f)) { err = "dx must be > 0 and lambda >= 0"; return PTY_ERR_INVALID_ARG; }
@@ -331,20 +310,32 @@ int validate_dims(const pty_dims* d, std::string& err) {
 Layout make_layout(const pty_dims& d) {
     Layout L{};
     const size_t NN = (size_t)d.N * d.N, B = (size_t)d.Bmax, M = (size_t)d.M, Nz = (size_t)d.Nz;
+    const size_t MT = M * (size_t)n_obj_of(d);       // waves per position: probe modes x object states
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
     L.probe_hat = take(M * NN * 8);
     L.prop = take(2 * (size_t)d.N * 8);
     L.I = take(B * NN * 4);
-    L.ws_psi = take(B * M * Nz * NN * 8);
-    L.ws_Psi = take(B * M * NN * 8);
-    L.ws_hat = take(save_hat_of(d) ? B * M * (Nz - 1) * NN * 8 : 0);
+    L.ws_psi = take(B * MT * Nz * NN * 8);
+    L.ws_Psi = take(B * MT * NN * 8);
+    L.ws_hat = take(save_hat_of(d) ? B * MT * (Nz - 1) * NN * 8 : 0);
     L.GP_hat = take(M * NN * 8);
     L.dsum = take(B * 4 * 4);
-    L.seed_w = take(d.N == 128 ? B * NN * 4 : 0);
+    L.seed_w = take(B * NN * 4);
     L.scalars = take(256);
+    L.stats = take(ST_COUNT * sizeof(double));
+    L.Isum = take(NN * 4);
+    L.Imsum = take(NN * 4);
+    L.taps = take(17 * 4);
+    L.gram = take(M * M * 16);
+    L.eigv = take(M * M * 16);
+    L.eigl = take(M * 8);
     const bool grads = d.flags & (PTY_FLAG_STEP | PTY_FLAG_HOST);
-    const size_t obj = Nz * (size_t)d.H * d.W * 8;
+    const size_t obj = (size_t)n_obj_of(d) * Nz * (size_t)d.H * d.W * 8;
+    const bool ap = d.flags & PTY_FLAG_AMP_PHASE;
+    L.ap_object = take(ap ? obj : 0);
+    L.ap_g_object = take(ap ? obj : 0);
+    L.ap_cnt = take(ap ? (size_t)d.H * d.W * 4 : 0);
     L.g_object = take(grads ? obj : 0);
     L.g_probe = take(grads ? M * NN * 8 : 0);
     L.g_pos = take(grads ? B * 2 * 4 : 0);
@@ -375,6 +366,8 @@ struct pty_plan {
     const void *f_object, *f_probe, *f_positions, *f_tilt, *f_meas;
     int32_t f_B;
 
+    pty_loss loss_cfg;           // pty_set_loss; mode 0 = plain amplitude sum
+    bool sparse_ready;           // the AP forward has put L_sparse into the statistics of this call
     // optional kernel timing (pty_profile)
     bool profiling;
     struct Timed { cudaEvent_t a, b; int which; };
@@ -384,6 +377,10 @@ struct pty_plan {
     double* d_loss() const { return at<double>(L.scalars); }
     int* d_flags() const { return at<int>(L.scalars + 64); }
     float* d_gdz() const { return at<float>(L.scalars + 128); }
+    double* d_stats() const { return at<double>(L.stats); }
+    int n_obj() const { return d.n_obj > 1 ? d.n_obj : 1; }
+    size_t object_elems() const { return (size_t)n_obj() * d.Nz * d.H * d.W; }
+    LossCfg loss_dev() const { return LossCfg{loss_cfg.w_gaussian, loss_cfg.w_poisson, loss_cfg.w_pacbed, loss_cfg.w_sparse, loss_cfg.eps}; }
 };
 
 namespace {
@@ -471,13 +468,13 @@ struct ScopedTimer {
 
 // N = 128 runs the two-items-per-CTA kernels (pty_kernels128g2.cuh); N = 64 and N = 256 the shared-memory passes
 template <class SH> cudaError_t launch_fwd_sh(pty_plan* p, const KArgs& A, cudaStream_t st) {
-    return launch(p, pty_fwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
+    return launch(p, pty_fwd_kernel<SH>, A.B * A.MT * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
 template <class SH> cudaError_t launch_bwd_sh(pty_plan* p, const KArgs& A, cudaStream_t st) {
-    return launch(p, pty_bwd_kernel<SH>, A.B * A.M * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
+    return launch(p, pty_bwd_kernel<SH>, A.B * A.MT * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
 int g2_grid(const pty_plan* p, const KArgs& A) {      // one persistent CTA per SM, or fewer when there is less work
-    const int pairs = (A.B * A.M + 1) / 2;
+    const int pairs = (A.B * A.MT + 1) / 2;
     return pairs < p->num_sms ? pairs : p->num_sms;
 }
 cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
@@ -505,6 +502,7 @@ KArgs make_args(const pty_plan* p, const void* object, const float* positions, c
     KArgs A{};
     const pty_dims& d = p->d;
     A.Nz = d.Nz; A.H = d.H; A.W = d.W; A.M = d.M; A.B = B;
+    A.Nobj = p->n_obj(); A.MT = d.M * A.Nobj;
     A.tilt_mode = d.tilt_mode;
     A.save_hat = save_hat_of(d) ? 1 : 0;
     A.dz = d.dz; A.lambda = d.lambda; A.dx = d.dx;
@@ -551,6 +549,16 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
     p->fwd_valid = false;
     PTY_CUDA(p, cudaMemsetAsync(loss, 0, sizeof(double), st));
     if (B == 0) return PTY_OK;
+    const bool paper_loss = p->loss_cfg.mode == 1;
+    if (paper_loss) {   // the minibatch sums of Eq. 5-7 (the AP entry point has already put L_sparse in place)
+        if (!p->sparse_ready) PTY_CUDA(p, cudaMemsetAsync(p->d_stats(), 0, ST_COUNT * sizeof(double), st));
+        else PTY_CUDA(p, cudaMemsetAsync(p->d_stats(), 0, 4 * sizeof(double), st));
+        if (p->loss_cfg.w_pacbed != 0.f) {
+            PTY_CUDA(p, cudaMemsetAsync(p->at<float>(p->L.Isum), 0, NN * sizeof(float), st));
+            PTY_CUDA(p, cudaMemsetAsync(p->at<float>(p->L.Imsum), 0, NN * sizeof(float), st));
+        }
+    }
+    p->sparse_ready = false;
     KArgs A = make_args(p, object, positions, tilt, meas, B);
     // a0: probe spectrum (unitary) and propagator factors
     if (d.N == 128)
@@ -562,10 +570,24 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
                            d.tilt_mode == 1 ? tilt : (const float*)nullptr, p->at<float2>(p->L.prop), p->at<float2>(p->L.prop) + d.N));
     PTY_CUDA(p, cudaMemsetAsync(A.I, 0, (size_t)B * NN * sizeof(float), st));
     PTY_CUDA(p, launch_fwd(p, A, st));
-    if (d.N == 128)
+    if (paper_loss) {
+        const LossCfg cfg = p->loss_dev();
+        float* Isum = p->at<float>(p->L.Isum);
+        float* Imsum = p->at<float>(p->L.Imsum);
+        if (d.N == 128) {
+            PTY_CUDA(p, launch(p, pty_loss_sums_kernel<true>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, cfg, p->d_stats(), loss_per_pos, Isum, Imsum, intensity));
+            PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss));
+            PTY_CUDA(p, launch(p, pty_seed_kernel<true>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, (int)B, cfg, (const double*)p->d_stats(), (const float*)Isum, (const float*)Imsum, A.seed_w));
+        } else {
+            PTY_CUDA(p, launch(p, pty_loss_sums_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, cfg, p->d_stats(), loss_per_pos, Isum, Imsum, (float*)nullptr));
+            PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss));
+            PTY_CUDA(p, launch(p, pty_seed_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, (int)B, cfg, (const double*)p->d_stats(), (const float*)Isum, (const float*)Imsum, A.seed_w));
+        }
+    } else if (d.N == 128) {
         PTY_CUDA(p, launch(p, pty_loss_seed128_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w, intensity));
-    else
-        PTY_CUDA(p, launch(p, pty_loss_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)NN, loss, loss_per_pos));
+    } else {
+        PTY_CUDA(p, launch(p, pty_loss_seed_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, loss, loss_per_pos, A.seed_w));
+    }
     if (intensity && d.N != 128)
         PTY_CUDA(p, cudaMemcpyAsync(intensity, A.I, (size_t)B * NN * sizeof(float), cudaMemcpyDeviceToDevice, st));
     p->fwd_valid = true;
@@ -577,14 +599,14 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
 // a7..a13 for one minibatch; needs the forward state
 int run_backward(pty_plan* p, const void* object, const float* positions, const float* tilt, const float* meas,
                  int32_t B, void* g_object, void* g_probe, float* g_positions, float* g_tilt, float* g_dz,
-                 int accumulate, cudaStream_t st) {
+                 int accumulate, cudaStream_t st, int accumulate_object = -1) {
+    // accumulate: add into g_probe, g_positions, g_tilt, g_dz; accumulate_object (default: the same) into g_object
     const pty_dims& d = p->d;
     const size_t NN = (size_t)d.N * d.N;
     p->last_stream = st;
-    if (!accumulate) {
-        PTY_CUDA(p, cudaMemsetAsync(g_object, 0, (size_t)d.Nz * d.H * d.W * sizeof(float2), st));
-        if (g_positions && B) PTY_CUDA(p, cudaMemsetAsync(g_positions, 0, (size_t)B * 2 * sizeof(float), st));
-    }
+    if (accumulate_object < 0) accumulate_object = accumulate;
+    if (!accumulate_object) PTY_CUDA(p, cudaMemsetAsync(g_object, 0, p->object_elems() * sizeof(float2), st));
+    if (!accumulate && g_positions && B) PTY_CUDA(p, cudaMemsetAsync(g_positions, 0, (size_t)B * 2 * sizeof(float), st));
     KArgs A = make_args(p, object, positions, tilt, meas, B);
     A.g_object = static_cast<float2*>(g_object);
     A.g_pos = g_positions;
@@ -659,6 +681,7 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
     if (!p) return fail(nullptr, PTY_ERR_INVALID_ARG, "out of host memory");
     p->d = *dims; p->L = L; p->ws = static_cast<unsigned char*>(workspace); p->device = device;
     p->last_stream = nullptr; p->launches = 0; p->fwd_valid = false; p->profiling = false;
+    p->loss_cfg = pty_loss{0, 1.f, 0.f, 0.f, 0.f, 1e-6f}; p->sparse_ready = false;
     int prev_device = -1;
     cudaError_t e = cudaGetDevice(&prev_device);
     if (e == cudaSuccess) e = cudaSetDevice(device);
@@ -797,7 +820,7 @@ int pty_step(pty_plan* plan, void* object, void* probe, float* positions, float*
     plan->fwd_valid = false;   // the parameters change below
     const size_t NN = (size_t)d.N * d.N;
     if ((rc = adam_launch(plan, (float*)object, (const float*)g_object, s->m_object, s->v_object,
-                          (size_t)d.Nz * d.H * d.W * 2, hp->lr_object, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+                          plan->object_elems() * 2, hp->lr_object, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
     if ((rc = adam_launch(plan, (float*)probe, (const float*)g_probe, s->m_probe, s->v_probe, (size_t)d.M * NN * 2,
                           hp->lr_probe, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
     if ((rc = adam_launch(plan, positions, g_pos, s->m_positions, s->v_positions, (size_t)B * 2, hp->lr_positions,
@@ -817,7 +840,7 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, con
     if (!(plan->d.flags & PTY_FLAG_HOST)) return fail(plan, PTY_ERR_INVALID_ARG, "plan was created without PTY_FLAG_HOST");
     const pty_dims& d = plan->d;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t NN = (size_t)d.N * d.N, obj_bytes = (size_t)d.Nz * d.H * d.W * 8, probe_bytes = (size_t)d.M * NN * 8;
+    const size_t NN = (size_t)d.N * d.N, obj_bytes = plan->object_elems() * 8, probe_bytes = (size_t)d.M * NN * 8;
     const size_t tilt_n = d.tilt_mode == 2 ? (size_t)B * 2 : 2;
     float2* dobj = plan->at<float2>(plan->L.h_object);
     float2* dprobe = plan->at<float2>(plan->L.h_probe);
@@ -845,6 +868,224 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, con
     if (h_g_tilt && dtilt) PTY_CUDA(plan, cudaMemcpyAsync(h_g_tilt, g_tilt, tilt_n * 4, cudaMemcpyDeviceToHost, st));
     PTY_CUDA(plan, cudaStreamSynchronize(st));
     return PTY_OK;
+}
+
+
+// ---------------------------------------------------------------------------- loss family (NEXT-2)
+int pty_set_loss(pty_plan* plan, const pty_loss* cfg) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    if (!cfg) { plan->loss_cfg = pty_loss{0, 1.f, 0.f, 0.f, 0.f, 1e-6f}; plan->fwd_valid = false; return PTY_OK; }
+    if (cfg->mode != 0 && cfg->mode != 1) return fail(plan, PTY_ERR_INVALID_ARG, "loss mode must be 0 or 1");
+    if (cfg->mode == 1 && !(cfg->eps > 0.f)) return fail(plan, PTY_ERR_INVALID_ARG, "Poisson eps must be > 0");
+    plan->loss_cfg = *cfg;
+    plan->fwd_valid = false;
+    return PTY_OK;
+}
+
+int pty_loss_terms(pty_plan* plan, double* terms4) {
+    if (!plan || !terms4) return PTY_ERR_INVALID_ARG;
+    DeviceGuard dg(plan->device);
+    PTY_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
+    PTY_CUDA(plan, cudaMemcpy(terms4, plan->d_stats() + ST_LG, 4 * sizeof(double), cudaMemcpyDeviceToHost));
+    return PTY_OK;
+}
+
+// ---------------------------------------------------------------------------- amplitude / phase object (NEXT-2)
+namespace {
+int grid_for(const pty_plan* p, size_t n) {
+    size_t blocks = (n + 255) / 256;
+    const size_t cap = (size_t)p->num_sms * 16;
+    return (int)(blocks < 1 ? 1 : blocks > cap ? cap : blocks);
+}
+
+int check_ap(pty_plan* p, const float* amp, const float* phase) {
+    if (!p) return PTY_ERR_INVALID_ARG;
+    if (!(p->d.flags & PTY_FLAG_AMP_PHASE)) return fail(p, PTY_ERR_INVALID_ARG, "plan was created without PTY_FLAG_AMP_PHASE");
+    if (!amp || !phase) return fail(p, PTY_ERR_INVALID_ARG, "amp or phase is null");
+    return PTY_OK;
+}
+
+// compose O = A exp(i phi), the coverage map of the minibatch and (loss mode 1) the sparsity term Eq. 8
+int ap_prepare(pty_plan* p, const float* amp, const float* phase, const float* positions, int32_t B, cudaStream_t st) {
+    const pty_dims& d = p->d;
+    const size_t n = p->object_elems(), HW = (size_t)d.H * d.W;
+    float2* obj = p->at<float2>(p->L.ap_object);
+    float* cnt = p->at<float>(p->L.ap_cnt);
+    PTY_CUDA(p, launch(p, pty_compose_object_kernel, grid_for(p, n), 256, 0, 1, st, amp, phase, obj, n));
+    const bool sparse = p->loss_cfg.mode == 1 && p->loss_cfg.w_sparse != 0.f;
+    if (p->loss_cfg.mode == 1) PTY_CUDA(p, cudaMemsetAsync(p->d_stats(), 0, ST_COUNT * sizeof(double), st));
+    if (sparse && B) {
+        PTY_CUDA(p, cudaMemsetAsync(cnt, 0, HW * sizeof(float), st));
+        PTY_CUDA(p, launch(p, pty_coverage_kernel, B, 256, 0, 1, st, positions, (int)d.N, (int)d.H, (int)d.W, cnt));
+        PTY_CUDA(p, launch(p, pty_sparse_sum_kernel, grid_for(p, n), 256, 0, 1, st, phase, (const float*)cnt, n, HW, p->d_stats()));
+        const double n_patch = (double)B * p->n_obj() * d.Nz * d.N * d.N;
+        PTY_CUDA(p, launch(p, pty_sparse_finalize_kernel, 1, 1, 0, 1, st, p->d_stats(), n_patch));
+    }
+    p->sparse_ready = p->loss_cfg.mode == 1;
+    return PTY_OK;
+}
+
+int ap_gradients(pty_plan* p, const float* amp, const float* phase, int32_t B, float* g_amp, float* g_phase,
+                 int accumulate, cudaStream_t st) {
+    const pty_dims& d = p->d;
+    const size_t n = p->object_elems(), HW = (size_t)d.H * d.W;
+    const bool sparse = p->loss_cfg.mode == 1 && p->loss_cfg.w_sparse != 0.f && B > 0;
+    const float c_sparse = sparse ? (float)((double)p->loss_cfg.w_sparse / ((double)B * p->n_obj() * d.Nz * d.N * d.N)) : 0.f;
+    PTY_CUDA(p, launch(p, pty_amp_phase_grad_kernel, grid_for(p, n), 256, 0, 1, st, (const float2*)p->at<float2>(p->L.ap_g_object),
+                       amp, phase, (const float*)p->at<float>(p->L.ap_cnt), c_sparse, n, HW, g_amp, g_phase, accumulate));
+    return PTY_OK;
+}
+}  // namespace
+
+int pty_forward_loss_ap(pty_plan* plan, const float* amp, const float* phase, const void* probe, const float* positions,
+                        const float* tilt, const float* meas_amp, int32_t B, double* loss, float* loss_per_pos,
+                        float* intensity, void* stream) {
+    int rc = check_ap(plan, amp, phase);
+    if (rc != PTY_OK) return rc;
+    float2* obj = plan->at<float2>(plan->L.ap_object);
+    rc = check_batch(plan, obj, probe, positions, tilt, meas_amp, B);
+    if (rc != PTY_OK) return rc;
+    if (!loss) return fail(plan, PTY_ERR_INVALID_ARG, "loss is null");
+    DeviceGuard dg(plan->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((rc = ap_prepare(plan, amp, phase, positions, B, st))) return rc;
+    rc = run_forward(plan, obj, probe, positions, tilt, meas_amp, B, loss, loss_per_pos, intensity, st);
+    plan->fwd_valid = false;       // the composed object is private: pty_backward_ap always runs its own forward
+    return rc;
+}
+
+int pty_backward_ap(pty_plan* plan, const float* amp, const float* phase, const void* probe, const float* positions,
+                    const float* tilt, const float* meas_amp, int32_t B, float* g_amp, float* g_phase, void* g_probe,
+                    float* g_positions, float* g_tilt, float* g_dz, int32_t flags, void* stream) {
+    int rc = check_ap(plan, amp, phase);
+    if (rc != PTY_OK) return rc;
+    float2* obj = plan->at<float2>(plan->L.ap_object);
+    rc = check_batch(plan, obj, probe, positions, tilt, meas_amp, B);
+    if (rc != PTY_OK) return rc;
+    if (!g_amp || !g_phase) return fail(plan, PTY_ERR_INVALID_ARG, "g_amp or g_phase is null");
+    if (g_dz && plan->d.Nz > 1 && !save_hat_of(plan->d))
+        return fail(plan, PTY_ERR_INVALID_ARG, "g_dz needs tilt_mode != 0 or PTY_FLAG_SPECTRA");
+    DeviceGuard dg(plan->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((rc = ap_prepare(plan, amp, phase, positions, B, st))) return rc;
+    if ((rc = run_forward(plan, obj, probe, positions, tilt, meas_amp, B, plan->d_loss(), nullptr, nullptr, st))) return rc;
+    plan->fwd_valid = false;
+    const int acc = (flags & PTY_BWD_ACCUMULATE) ? 1 : 0;
+    // the complex gradient of THIS minibatch goes to the workspace (never accumulated there); amp / phase accumulate
+    if ((rc = run_backward(plan, obj, positions, tilt, meas_amp, B, plan->at<float2>(plan->L.ap_g_object), g_probe,
+                           g_positions, g_tilt, g_dz, acc, st, 0))) return rc;
+    return ap_gradients(plan, amp, phase, B, g_amp, g_phase, acc, st);
+}
+
+int pty_step_ap(pty_plan* plan, float* amp, float* phase, void* probe, float* positions, float* tilt, const float* meas_amp,
+                int32_t B, const pty_adam_ap* hp, const pty_adam_state_ap* s, double* loss, void* stream) {
+    int rc = check_ap(plan, amp, phase);
+    if (rc != PTY_OK) return rc;
+    float2* obj = plan->at<float2>(plan->L.ap_object);
+    rc = check_batch(plan, obj, probe, positions, tilt, meas_amp, B);
+    if (rc != PTY_OK) return rc;
+    if (!hp || !s || !loss) return fail(plan, PTY_ERR_INVALID_ARG, "hp, st or loss is null");
+    if (!(plan->d.flags & PTY_FLAG_STEP)) return fail(plan, PTY_ERR_INVALID_ARG, "plan was created without PTY_FLAG_STEP");
+    DeviceGuard dg(plan->device);
+    const pty_dims& d = plan->d;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // the step's real gradient buffers: g_amp and g_phase share the STEP buffer reserved for a complex g_object
+    float* g_amp = plan->at<float>(plan->L.g_object);
+    float* g_phase = g_amp + plan->object_elems();
+    float2* g_probe = plan->at<float2>(plan->L.g_probe);
+    float* g_pos = plan->at<float>(plan->L.g_pos);
+    float* g_tilt = plan->at<float>(plan->L.g_tilt);
+    if ((rc = ap_prepare(plan, amp, phase, positions, B, st))) return rc;
+    if ((rc = run_forward(plan, obj, probe, positions, tilt, meas_amp, B, loss, nullptr, nullptr, st))) return rc;
+    const bool tilt_on = d.tilt_mode != 0 && hp->lr_tilt != 0.f;
+    if ((rc = run_backward(plan, obj, positions, tilt, meas_amp, B, plan->at<float2>(plan->L.ap_g_object),
+                           hp->lr_probe != 0.f ? g_probe : nullptr, hp->lr_positions != 0.f ? g_pos : nullptr,
+                           tilt_on ? g_tilt : nullptr, nullptr, 0, st))) return rc;
+    plan->fwd_valid = false;
+    if ((rc = ap_gradients(plan, amp, phase, B, g_amp, g_phase, 0, st))) return rc;
+    const size_t NN = (size_t)d.N * d.N, n = plan->object_elems();
+    if ((rc = adam_launch(plan, amp, g_amp, s->m_amp, s->v_amp, n, hp->lr_amp, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    if ((rc = adam_launch(plan, phase, g_phase, s->m_phase, s->v_phase, n, hp->lr_phase, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    if ((rc = adam_launch(plan, (float*)probe, (const float*)g_probe, s->m_probe, s->v_probe, (size_t)d.M * NN * 2,
+                          hp->lr_probe, hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    if ((rc = adam_launch(plan, positions, g_pos, s->m_positions, s->v_positions, (size_t)B * 2, hp->lr_positions,
+                          hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    if (tilt_on)
+        if ((rc = adam_launch(plan, tilt, g_tilt, s->m_tilt, s->v_tilt, d.tilt_mode == 2 ? (size_t)B * 2 : 2, hp->lr_tilt,
+                              hp->beta1, hp->beta2, hp->eps, hp->t, st))) return rc;
+    return PTY_OK;
+}
+
+// ---------------------------------------------------------------------------- constraints (NEXT-3)
+namespace {
+// Eq. 13 on a float array viewed as [outer][Nz][plane]
+int rz_filter_launch(pty_plan* p, float* x, size_t outer, size_t plane, float sigma_z, cudaStream_t st) {
+    const int Nz = p->d.Nz;
+    if (!(sigma_z > 0.f) || Nz < 2) return PTY_OK;
+    const int R = std::max(1, (int)std::ceil(2.0 * (double)sigma_z));
+    if (R > 8) return fail(p, PTY_ERR_UNSUPPORTED, "r_z filter: sigma_z = %g needs a radius of %d slices (max 8)", (double)sigma_z, R);
+    float taps[17];
+    double sum = 0.0;
+    for (int j = -R; j <= R; ++j) sum += std::exp(-(double)j * j / (2.0 * (double)sigma_z * sigma_z));
+    for (int j = -R; j <= R; ++j) taps[j + R] = (float)(std::exp(-(double)j * j / (2.0 * (double)sigma_z * sigma_z)) / sum);
+    float* dtaps = p->at<float>(p->L.taps);
+    // the taps travel as kernel-parameter-sized data through a stream-ordered copy from a pageable host buffer
+    // (copied by the driver before the call returns)
+    PTY_CUDA(p, cudaMemcpyAsync(dtaps, taps, (2 * R + 1) * sizeof(float), cudaMemcpyHostToDevice, st));
+    const size_t columns = outer * plane;
+    const int grid = grid_for(p, columns);
+    cudaError_t e = cudaSuccess;
+    switch (R) {
+#define PTY_RZ(RR) case RR: e = launch(p, pty_rz_filter_kernel<RR>, grid, 256, 0, 1, st, x, Nz, plane, columns, (const float*)dtaps); break;
+        PTY_RZ(1) PTY_RZ(2) PTY_RZ(3) PTY_RZ(4) PTY_RZ(5) PTY_RZ(6) PTY_RZ(7) PTY_RZ(8)
+#undef PTY_RZ
+    }
+    PTY_CUDA(p, e);
+    return PTY_OK;
+}
+}  // namespace
+
+int pty_constrain(pty_plan* plan, float* amp, float* phase, void* probe, const pty_constraints* c, void* stream) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    if (!c) return fail(plan, PTY_ERR_INVALID_ARG, "constraints is null");
+    DeviceGuard dg(plan->device);
+    const pty_dims& d = plan->d;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    plan->last_stream = st;
+    plan->fwd_valid = false;
+    int rc;
+    const size_t n = plan->object_elems(), HW = (size_t)d.H * d.W;
+    if (c->sigma_z > 0.f) {
+        if (amp && (rc = rz_filter_launch(plan, amp, (size_t)plan->n_obj(), HW, c->sigma_z, st))) return rc;
+        if (phase && (rc = rz_filter_launch(plan, phase, (size_t)plan->n_obj(), HW, c->sigma_z, st))) return rc;
+    }
+    const int pos = c->phase_positive && phase, clamp = c->clamp_amp && amp;
+    if (clamp && !(c->amp_min <= c->amp_max)) return fail(plan, PTY_ERR_INVALID_ARG, "amp_min > amp_max");
+    if (pos || clamp)
+        PTY_CUDA(plan, launch(plan, pty_clip_clamp_kernel, grid_for(plan, n), 256, 0, 1, st, amp, phase, n, pos, clamp, c->amp_min, c->amp_max));
+    if (c->ortho_probe) {
+        if (!probe) return fail(plan, PTY_ERR_INVALID_ARG, "ortho_probe needs the probe");
+        if (d.M > kMaxModes) return fail(plan, PTY_ERR_UNSUPPORTED, "probe orthogonalisation supports M <= %d", kMaxModes);
+        const size_t NN = (size_t)d.N * d.N;
+        double2* G = plan->at<double2>(plan->L.gram);
+        double2* V = plan->at<double2>(plan->L.eigv);
+        double* lam = plan->at<double>(plan->L.eigl);
+        PTY_CUDA(plan, launch(plan, pty_gram_kernel, d.M * (d.M + 1) / 2, 256, 0, 1, st, (const float2*)probe, (int)d.M, NN, G));
+        PTY_CUDA(plan, launch(plan, pty_eigh_kernel, 1, 32, 0, 1, st, (const double2*)G, (int)d.M, V, lam));
+        PTY_CUDA(plan, launch(plan, pty_mix_modes_kernel, grid_for(plan, NN), 256, 0, 1, st, (float2*)probe, (int)d.M, NN, (const double2*)V));
+    }
+    return PTY_OK;
+}
+
+int pty_rz_filter_object(pty_plan* plan, void* object, float sigma_z, void* stream) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    if (!object) return fail(plan, PTY_ERR_INVALID_ARG, "object is null");
+    DeviceGuard dg(plan->device);
+    plan->last_stream = static_cast<cudaStream_t>(stream);
+    plan->fwd_valid = false;
+    // complex64 = interleaved (re, im): a plane of H W complex values is 2 H W floats
+    return rz_filter_launch(plan, static_cast<float*>(object), (size_t)plan->n_obj(), (size_t)plan->d.H * plan->d.W * 2, sigma_z,
+                            static_cast<cudaStream_t>(stream));
 }
 
 int pty_status(pty_plan* plan, int32_t* device_flags) {

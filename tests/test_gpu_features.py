@@ -1,0 +1,301 @@
+"""GPU parity for the rows SURVEY.md §8(f) marks "next": the paper's loss family Eq. 5-9 and the amplitude / phase
+object (NEXT-2), the per-iteration constraints (NEXT-3),
+mixed object states (NEXT-4) -- each against oracle/losses.py / oracle/constraints.py through the
+C ABI, at the north_star tolerances -- and CUDA-graph capture of the enqueue-only calls."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import oracle  # noqa: E402
+from oracle import constraints as oc  # noqa: E402
+from oracle import losses as ol  # noqa: E402
+from cases import geom_of, make_case, rel_l2  # noqa: E402
+from paper_2505_07814_b200 import synth  # noqa: E402
+
+LOSS_RTOL, GRAD_RTOL = 1e-4, 1e-3
+
+
+@pytest.fixture(scope="module")
+def pty():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2505_07814_b200 import build
+    build.build()
+    from paper_2505_07814_b200 import binding
+    return binding
+
+
+def dev(x):
+    return None if x is None else torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def small_case(c, B, which="A", **over):
+    cfg = synth.get_config(c, **over)
+    idx = synth.minibatch(cfg, 0, cfg.B)[:B]
+    case = make_case(c, which, idx)
+    if over:
+        M, Nz = cfg.M, cfg.Nz
+        case = dict(case, cfg=cfg, object=np.ascontiguousarray(case["object"][:Nz]), probe=np.ascontiguousarray(case["probe"][:M]))
+        tr = synth.truth(synth.get_config(c))
+        I_true = oracle.intensity_batch(tr["object"][:Nz], tr["probe"][:M], tr["positions"][idx],
+                                        tr["tilt"] if cfg.tilt_mode else None, geom_of(cfg))
+        case["meas"] = synth.poisson_amplitudes(cfg, I_true, idx)
+    return case
+
+
+CASES = {"c1": lambda: small_case(1, 12), "c3": lambda: small_case(3, 5, Nz=3, M=3), "c5": lambda: small_case(5, 2, Nz=2, M=2)}
+WEIGHTS = {"gaussian": ol.LossWeights(1, 0, 0, 0), "poisson": ol.LossWeights(0, 1, 0, 0),
+           "pacbed": ol.LossWeights(0, 0, 1, 0), "total": ol.LossWeights(1.0, 0.4, 0.6, 0.0)}
+
+
+@pytest.mark.parametrize("name", ["c1", "c3", "c5"])
+@pytest.mark.parametrize("wname", list(WEIGHTS))
+def test_paper_loss_family_complex_object(pty, name, wname):
+    """Eq. 5, 6, 7 and their weighted total (Eq. 9) as the loss of pty_forward_loss / pty_backward: value, the three
+    terms and every gradient against the oracle.  N = 64, 128 (thread-order intensities) and 256 (cluster path)."""
+    case, w = CASES[name](), WEIGHTS[wname]
+    cfg = case["cfg"]
+    B = len(case["positions"])
+    ref = ol.total_loss_and_gradients(case["object"], case["probe"], case["positions"], case["tilt"], case["meas"],
+                                      geom_of(cfg), w)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, tilt_mode=case["tilt_mode"],
+                    flags=pty.PTY_FLAG_SPECTRA)
+    plan.set_loss(1, w.gaussian, w.poisson, w.pacbed, 0.0, w.eps)
+    obj, probe, pos, tilt, meas = dev(case["object"]), dev(case["probe"]), dev(case["positions"]), dev(case["tilt"]), dev(case["meas"])
+    inten = torch.zeros(B, cfg.N, cfg.N, device="cuda")
+    loss = plan.forward_loss(obj, probe, pos, tilt, meas, intensity=inten)
+    g_obj, g_probe = torch.zeros_like(obj), torch.zeros_like(probe)
+    g_pos = torch.zeros(B, 2, device="cuda")
+    g_tilt = torch.zeros(2, device="cuda") if case["tilt_mode"] else None
+    g_dz = torch.zeros(1, device="cuda") if cfg.Nz > 1 else None
+    plan.backward(obj, probe, pos, tilt, meas, g_obj, g_probe, g_pos, g_tilt, g_dz, flags=pty.PTY_BWD_REUSE_FORWARD)
+    assert plan.status()[0] == 0
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
+    terms = plan.loss_terms()
+    for k in ("gaussian", "poisson"):                 # always evaluated; PACBED only when it carries a weight
+        assert abs(terms[k] - ref["terms"][k]) <= LOSS_RTOL * abs(ref["terms"][k]), (k, terms, ref["terms"])
+    if w.pacbed != 0.0:
+        assert abs(terms["pacbed"] - ref["terms"]["pacbed"]) <= LOSS_RTOL * abs(ref["terms"]["pacbed"]), (terms, ref["terms"])
+    assert np.max(np.abs(inten.cpu().numpy() - ref["intensity"])) <= 1e-4 * ref["intensity"].max()
+    errs = {"g_object": rel_l2(g_obj.cpu().numpy(), ref["g_object"]), "g_probe": rel_l2(g_probe.cpu().numpy(), ref["g_probe"]),
+            "g_positions": rel_l2(g_pos.cpu().numpy(), ref["g_positions"])}
+    if g_tilt is not None:
+        errs["g_tilt"] = rel_l2(g_tilt.cpu().numpy(), ref["g_tilt"].sum(0))
+    if g_dz is not None:
+        errs["g_dz"] = abs(g_dz.item() - ref["g_dz"]) / abs(ref["g_dz"])
+    print(name, wname, f"loss {loss.item():.6g}", " ".join(f"{k} {v:.2e}" for k, v in errs.items()))
+    assert all(v <= GRAD_RTOL for v in errs.values()), errs
+    # back to the default loss: the plain sum again
+    plan.set_loss(0)
+    L0 = plan.forward_loss(obj, probe, pos, tilt, meas).item()
+    S = oracle.forward_loss_batch(case["object"], case["probe"], case["positions"], case["tilt"], case["meas"], geom_of(cfg))[0]
+    assert abs(L0 - S) <= LOSS_RTOL * S
+
+
+def _amp_phase_of(obj):
+    return np.abs(obj).astype(np.float32), np.angle(obj).astype(np.float32)
+
+
+@pytest.mark.parametrize("name", ["c1", "c3"])
+def test_amplitude_phase_object_with_sparsity(pty, name):
+    """O = A exp(i phi) with the full Eq. 9 including the L1 sparsity of the phase patches (Eq. 8):
+    loss, terms, g_amp, g_phase and the other gradients; then accumulation over two half batches."""
+    case = CASES[name]()
+    cfg = case["cfg"]
+    B = len(case["positions"])
+    amp, phase = _amp_phase_of(case["object"])
+    w = ol.LossWeights(1.0, 0.4, 0.6, 0.1)
+    ref = ol.total_loss_and_gradients(None, case["probe"], case["positions"], case["tilt"], case["meas"], geom_of(cfg), w,
+                                      amp=amp, phase=phase)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, tilt_mode=case["tilt_mode"],
+                    flags=pty.PTY_FLAG_AMP_PHASE)
+    plan.set_loss(1, w.gaussian, w.poisson, w.pacbed, w.sparse, w.eps)
+    tA, tp, probe, pos, meas = dev(amp), dev(phase), dev(case["probe"]), dev(case["positions"]), dev(case["meas"])
+    loss = plan.forward_loss_ap(tA, tp, probe, pos, None, meas)
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
+    terms = plan.loss_terms()
+    assert abs(terms["sparse"] - ref["terms"]["sparse"]) <= LOSS_RTOL * ref["terms"]["sparse"]
+    gA, gp = torch.full_like(tA, 7.0), torch.full_like(tp, 7.0)
+    g_probe, g_pos = torch.zeros_like(probe), torch.zeros(B, 2, device="cuda")
+    plan.backward_ap(tA, tp, probe, pos, None, meas, gA, gp, g_probe, g_pos)
+    errs = {"g_amp": rel_l2(gA.cpu().numpy(), ref["g_amp"]), "g_phase": rel_l2(gp.cpu().numpy(), ref["g_phase"]),
+            "g_probe": rel_l2(g_probe.cpu().numpy(), ref["g_probe"]), "g_positions": rel_l2(g_pos.cpu().numpy(), ref["g_positions"])}
+    print(name, "amp/phase", " ".join(f"{k} {v:.2e}" for k, v in errs.items()))
+    assert all(v <= GRAD_RTOL for v in errs.values()), errs
+    # the sparsity gradient alone (data weights 0): w4 count sign(phase) / n_patch, exact up to float32 rounding
+    plan.set_loss(1, 0.0, 0.0, 0.0, 1.0, w.eps)
+    plan.backward_ap(tA, tp, probe, pos, None, meas, gA, gp)
+    _, g_s = ol.sparse_term(phase, case["positions"], cfg.N)
+    assert rel_l2(gp.cpu().numpy(), g_s) <= 1e-5 and float(gA.abs().max()) == 0.0
+
+
+def test_step_ap_is_the_papers_update(pty):
+    """pty_step_ap: Eq. 9 loss (NRMSE + 0.1 L1 sparsity), Adam with separate learning rates on amplitude,
+    phase, probe and positions.  First step from zero moments against the oracle's gradients + oracle.adam_step."""
+    case = CASES["c3"]()
+    cfg = case["cfg"]
+    B = len(case["positions"])
+    amp, phase = _amp_phase_of(case["object"])
+    w = ol.LossWeights(1.0, 0.0, 0.0, 0.1)
+    ref = ol.total_loss_and_gradients(None, case["probe"], case["positions"], None, case["meas"], geom_of(cfg), w, amp=amp, phase=phase)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, flags=pty.PTY_FLAG_AMP_PHASE | pty.PTY_FLAG_STEP)
+    plan.set_loss(1, w.gaussian, w.poisson, w.pacbed, w.sparse, w.eps)
+    tA, tp, probe, pos, meas = dev(amp), dev(phase), dev(case["probe"]), dev(case["positions"]), dev(case["meas"])
+    state = {}
+    for nm, t in (("amp", tA), ("phase", tp), ("probe", probe), ("positions", pos)):
+        n = t.numel() * (2 if t.is_complex() else 1)
+        state["m_" + nm], state["v_" + nm] = torch.zeros(n, device="cuda"), torch.zeros(n, device="cuda")
+    lr = {"amp": 5e-4, "phase": 5e-4, "probe": 1e-4, "positions": 5e-4}
+    hp = pty.pty_adam_ap(lr["amp"], lr["phase"], lr["probe"], lr["positions"], 0.0, 0.9, 0.999, 1e-8, 1)
+    loss = plan.step_ap(tA, tp, probe, pos, None, meas, hp, state)
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
+    for nm, before, g, t in (("amp", amp, ref["g_amp"], tA), ("phase", phase, ref["g_phase"], tp)):
+        new, m1, _ = oracle.adam_step(before, g, np.zeros(before.size), np.zeros(before.size), 1, lr[nm])
+        big = np.abs(g) > 1e-3 * np.abs(g).max()                     # |g| >> eps: the step is -lr sign(g)
+        d_gpu = t.cpu().numpy().astype(np.float64) - before
+        np.testing.assert_allclose(d_gpu[big], (new.reshape(before.shape) - before)[big], rtol=2e-3, atol=2e-7)
+        assert rel_l2(state["m_" + nm].cpu().numpy().reshape(before.shape), m1.reshape(before.shape)) <= GRAD_RTOL
+
+
+@pytest.mark.parametrize("name", ["c1", "c3"])
+def test_mixed_object_states(pty, name):
+    """Eq. 2 with N = 2 object states: I = sum_m sum_n |.|^2; object and g_object are [2][Nz][H][W]."""
+    case = CASES[name]()
+    cfg = case["cfg"]
+    B = len(case["positions"])
+    rng = np.random.default_rng(17)
+    second = case["object"] * np.exp(1j * 0.1 * rng.standard_normal(case["object"].shape)).astype(np.complex64)
+    obj2 = np.ascontiguousarray(np.stack([case["object"], second * 0.6]).astype(np.complex64))
+    geom = geom_of(cfg)
+    idx = case["indices"]
+    tr = synth.truth(synth.get_config(cfg.c))
+    tobj = np.stack([tr["object"][:cfg.Nz], 0.6 * tr["object"][:cfg.Nz]])
+    meas = synth.poisson_amplitudes(cfg, ol.intensity_batch_states(tobj, tr["probe"][:cfg.M], tr["positions"][idx], None, geom), idx)
+    for mode, w in ((0, None), (1, ol.LossWeights(1.0, 0.4, 0.6, 0.0))):
+        plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, n_obj=2)
+        if mode == 1:
+            plan.set_loss(1, w.gaussian, w.poisson, w.pacbed, 0.0, w.eps)
+            ref = ol.total_loss_and_gradients(obj2, case["probe"], case["positions"], None, meas, geom, w)
+        else:
+            # plain sum with two states: the seed needs the SUMMED intensity, dS/dI = 1 - a / sqrt(I)
+            I = ol.intensity_batch_states(obj2, case["probe"], case["positions"], None, geom)
+            ref = _plain_sum_states(obj2, case["probe"], case["positions"], meas, geom, I)
+        o, probe, pos, dm = dev(obj2), dev(case["probe"]), dev(case["positions"]), dev(meas)
+        inten = torch.zeros(B, cfg.N, cfg.N, device="cuda")
+        loss = plan.forward_loss(o, probe, pos, None, dm, intensity=inten)
+        g_obj, g_probe, g_pos = torch.zeros_like(o), torch.zeros_like(probe), torch.zeros(B, 2, device="cuda")
+        plan.backward(o, probe, pos, None, dm, g_obj, g_probe, g_pos, flags=pty.PTY_BWD_REUSE_FORWARD)
+        assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
+        assert np.max(np.abs(inten.cpu().numpy() - ref["intensity"])) <= 1e-4 * ref["intensity"].max()
+        for n in range(2):
+            assert rel_l2(g_obj[n].cpu().numpy(), ref["g_object"][n]) <= GRAD_RTOL, (mode, n)
+        assert rel_l2(g_probe.cpu().numpy(), ref["g_probe"]) <= GRAD_RTOL
+        assert rel_l2(g_pos.cpu().numpy(), ref["g_positions"]) <= GRAD_RTOL
+
+
+def _plain_sum_states(obj, probe, positions, meas, geom, I):
+    """Oracle for the plain amplitude sum with object states: S = sum (sqrt(I) - a)^2, dS/dI = 1 - a / sqrt(I)."""
+    a = np.asarray(meas, np.float64)
+    sq = np.sqrt(I)
+    dLdI = np.where(I > 0, 1.0 - a / np.where(I > 0, sq, 1.0), 0.0)
+    g_obj = np.zeros(obj.shape, np.complex128)
+    g_probe = np.zeros(probe.shape, np.complex128)
+    g_pos = np.zeros((len(positions), 2))
+    for b in range(len(positions)):
+        for n in range(obj.shape[0]):
+            f = oracle.forward_position(obj[n], probe, positions[b], (0.0, 0.0), geom)
+            gp, _, _ = oracle.backprop_position(f, probe, dLdI[b], (0.0, 0.0), geom, g_obj[n], g_probe)
+            g_pos[b] += gp
+    return {"loss": float(np.sum((sq - a) ** 2)), "intensity": I, "g_object": g_obj, "g_probe": g_probe, "g_positions": g_pos}
+
+
+# ----------------------------------------------------------------------------- constraints (NEXT-3)
+def test_probe_orthogonalisation(pty):
+    """Unique parts compared exactly (powers, density operator, orthogonality); each mode up to its unit phase."""
+    cfg = synth.get_config(4)
+    rng = np.random.default_rng(5)
+    mix = rng.standard_normal((cfg.M, cfg.M)) + 1j * rng.standard_normal((cfg.M, cfg.M))
+    P = np.tensordot(mix, synth.make_probe(cfg), axes=1).astype(np.complex64)      # strongly non-orthogonal modes
+    Q_ref, lam_ref = oc.orthogonalize_modes(P)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, 4, cfg.dz, cfg.lam, cfg.dx)
+    t = dev(P)
+    plan.constrain(probe=t, ortho_probe=True)
+    Q = t.cpu().numpy().astype(np.complex128)
+    qf = Q.reshape(cfg.M, -1)
+    G = np.conj(qf) @ qf.T
+    lam = np.real(np.diag(G))
+    np.testing.assert_allclose(lam, lam_ref, rtol=1e-4, atol=1e-6 * lam_ref[0])
+    assert np.max(np.abs(G - np.diag(lam))) <= 1e-5 * lam_ref[0]                     # mutually orthogonal
+    x = rng.standard_normal(qf.shape[1]) + 1j * rng.standard_normal(qf.shape[1])   # density operator on a test vector
+    rho = lambda modes: modes.T @ (np.conj(modes) @ x)
+    assert rel_l2(rho(qf), rho(P.reshape(cfg.M, -1).astype(np.complex128))) <= 1e-5
+    for k in range(cfg.M):
+        if lam_ref[k] < 1e-4 * lam_ref[0]:
+            continue
+        ph = np.vdot(Q_ref[k], Q[k])
+        assert rel_l2(Q[k], Q_ref[k] * ph / abs(ph)) <= 1e-3 * max(1.0, lam_ref[0] / lam_ref[k]) ** 0.5, k
+
+
+def test_rz_filter_positivity_and_amplitude_clamp(pty):
+    cfg = synth.get_config(3)
+    obj = synth.eval_point(cfg, "A")["object"]
+    rng = np.random.default_rng(2)
+    amp = (np.abs(obj) + 0.05 * rng.standard_normal(obj.shape)).astype(np.float32)
+    phase = (np.angle(obj) - 0.1).astype(np.float32)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, 4, cfg.dz, cfg.lam, cfg.dx)
+    for sigma in (1.0, 0.4, 2.3):
+        tA, tp, to = dev(amp), dev(phase), dev(obj)
+        plan.constrain(amp=tA, phase=tp, sigma_z=sigma)
+        np.testing.assert_allclose(tA.cpu().numpy(), oc.rz_filter(amp, sigma), rtol=2e-6, atol=2e-7)
+        np.testing.assert_allclose(tp.cpu().numpy(), oc.rz_filter(phase, sigma), rtol=2e-6, atol=2e-7)
+        plan.rz_filter_object(to, sigma)
+        assert rel_l2(to.cpu().numpy(), oc.rz_filter(obj, sigma)) <= 1e-6
+    tA, tp = dev(amp), dev(phase)
+    plan.constrain(amp=tA, phase=tp, sigma_z=1.0, phase_positive=True, clamp_amp=(0.98, 1.02))   # the paper's set (:539)
+    ref_p = oc.clip_phase_positive(oc.rz_filter(phase, 1.0))
+    ref_a = oc.clamp_amplitude(oc.rz_filter(amp, 1.0))
+    np.testing.assert_allclose(tp.cpu().numpy(), ref_p, rtol=2e-6, atol=2e-7)
+    np.testing.assert_allclose(tA.cpu().numpy(), ref_a, rtol=2e-6, atol=2e-7)
+    assert float(tp.min()) >= 0.0 and float(tA.min()) >= 0.98 and float(tA.max()) <= 1.02
+    with pytest.raises(pty.PtyError):
+        plan.constrain(amp=tA, sigma_z=9.0)                                                     # radius > 8 slices
+
+
+# ----------------------------------------------------------------------------- CUDA graphs
+def test_forward_backward_can_be_captured_in_a_cuda_graph(pty):
+    """The enqueue-only calls neither allocate nor synchronise: one forward + gradient pass on fixed pointers is
+    recorded with stream capture and replayed (the launch-bound small configurations, c1)."""
+    case = CASES["c1"]()
+    cfg = case["cfg"]
+    B = len(case["positions"])
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx)
+    obj, probe, pos, meas = dev(case["object"]), dev(case["probe"]), dev(case["positions"]), dev(case["meas"])
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    g_obj, g_probe, g_pos = torch.zeros_like(obj), torch.zeros_like(probe), torch.zeros(B, 2, device="cuda")
+
+    def run():
+        plan.forward_loss(obj, probe, pos, None, meas, loss)
+        plan.backward(obj, probe, pos, None, meas, g_obj, g_probe, g_pos, flags=pty.PTY_BWD_REUSE_FORWARD)
+
+    run()
+    torch.cuda.synchronize()
+    eager = (loss.item(), g_obj.clone(), g_probe.clone())
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        run()
+    torch.cuda.current_stream().wait_stream(side)
+    with torch.cuda.graph(graph):
+        run()
+    g_obj.zero_(); loss.zero_()
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    ref = oracle.grad_batch(case["object"], case["probe"], case["positions"], None, case["meas"], geom_of(cfg))
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * ref["loss"]
+    assert rel_l2(g_obj.cpu().numpy(), ref["g_object"]) <= GRAD_RTOL
+    assert rel_l2(g_obj.cpu().numpy(), eager[1].cpu().numpy()) <= 1e-5
+    assert plan.status()[0] == 0

@@ -515,4 +515,5 @@ def test_pty_step_with_global_tilt_on_multislice(pty):
     big = np.abs(gp) > 1e-3 * np.abs(gp).max()
     d_gpu = probe.cpu().numpy().astype(np.complex128).view(np.float64) - ev["probe"].astype(np.complex128).view(np.float64)
     d_ref = new_probe.reshape(ev["probe"].shape).view(np.float64) - ev["probe"].astype(np.complex128).view(np.float64)
-    np.testing.assert_allclose(d_gpu[big], d_ref[big], rtol=2e-3, atol=1e-4 * np.abs(d_ref).max())
+    # probe values reach ~10 in float32 (ulp 1e-6): the 1e-4 step is resolved to about 1 %
+    np.testing.assert_allclose(d_gpu[big], d_ref[big], rtol=2e-3, atol=2e-6)
