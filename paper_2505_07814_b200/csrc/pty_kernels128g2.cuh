@@ -22,11 +22,36 @@
 #include "pty_fft128.cuh"
 #include "pty_kernels.cuh"
 
+#ifndef PTY_G2_EARLY
+#define PTY_G2_EARLY 0  // request the first D saved-wave chunks before the park phase's inverse transforms
+#endif
 #ifndef PTY_G2_D
 #define PTY_G2_D 3      // chunks of saved-wave / object rows in flight in the adjoint's streaming step
 #endif
 
 namespace pty {
+
+// timing ablations (never defined in the product build): drop one memory stream of the adjoint's streaming step
+PTY_DEV void g2_red_obj(float2* p, float2 v) {
+#ifdef PTY_ABL_RED
+    if (v.x == 1.2345e-30f)
+#endif
+    red_add2(p, v);
+}
+PTY_DEV float4 g2_ld_psi(const float4* p) {
+#ifdef PTY_ABL_PSI
+    return make_float4(1.f, 2.f, 3.f, 0.5f);
+#else
+    return ld_stream4_pinned(p);
+#endif
+}
+PTY_DEV float2 g2_ld_obj(const float2* p) {
+#ifdef PTY_ABL_OBJ
+    return make_float2(0.9f, 0.1f);
+#else
+    return ldg2_pinned(p);
+#endif
+}
 
 struct G2Smem {
     static constexpr size_t xch_bytes = F128::xch_bytes;
@@ -50,8 +75,13 @@ struct G2 {
         tmem_fence_after_sync();
     }
     PTY_DEV void grp_sync() const { asm volatile("bar.sync %0, 256;" ::"r"(9 + G) : "memory"); }
+#ifdef PTY_ABL_ONEGROUP      // timing ablation: group 1 idles, group 0 owns the transpose buffer
+    PTY_DEV void acquireX() const {}
+    PTY_DEV void releaseX() const {}
+#else
     PTY_DEV void acquireX() const { asm volatile("bar.sync %0, 512;" ::"r"(11 + G) : "memory"); }
     PTY_DEV void releaseX() const { asm volatile("bar.arrive %0, 512;" ::"r"(11 + (G ^ 1)) : "memory"); }
+#endif
 };
 
 PTY_DEV G2 make_g2(unsigned char* smem) {
@@ -215,10 +245,12 @@ PTY_DEV void g2_accumulate(const G2& c, int slot, float v) {
 }
 
 // ------------------------------------------------------------------------------ forward (a2-a5)
-// item = b M + m; live = false for the padding item of an odd grid (same control flow, no global writes).
+// item = b MT + n M + m.  The padding item of an odd item count is a GHOST: it runs item n - 1 again with its probe
+// (forward) or its seed (adjoint) scaled by 0 and its saved waves in the spare slot `ghost_slot` of the workspace, so
+// that every reduction it issues adds zero and no store, reduction or load in these bodies needs a predicate.
 // HAT: keep the propagated spectra (tilt / dz gradients); a compile-time switch so that the common no-tilt kernels
 // carry neither the code nor the registers of that path.
-template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
+template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, int slot, float scl) {
     constexpr int N = 128, NT = F128::NT;
     int b, m;
     size_t obj_off;
@@ -227,7 +259,7 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
     setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
     c.grp_sync();
     const size_t NN = (size_t)N * N;
-    const size_t bm = (size_t)item;
+    const size_t bm = (size_t)slot;
     float2 v[32];
     NoBg bg;
     {   // a2 (K): E . P^ -> inverse x radix-4 -> role blocks
@@ -237,7 +269,7 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
             const int o = 2 * c.gg + h;
             const float2* Ph = A.probe_hat + (size_t)m * NN + 128 * o + c.c;
 #pragma unroll
-            for (int r = 0; r < 32; ++r) v[r] = cmul(cmul(ldg2(Ph + r * NT), ey), c.Ex[c.kx(o, r)]);
+            for (int r = 0; r < 32; ++r) v[r] = cmul(cmul(cscale(ldg2(Ph + r * NT), scl), ey), c.Ex[c.kx(o, r)]);
             g2_radix4<+1>(c, o, v);
             g2_st_slots(c, o, v);
         }
@@ -264,7 +296,7 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
                 if (J < 3) { _Pragma("unroll") for (int i = 0; i < 8; ++i)                              \
                     NXT[i] = ldg2_pinned(obj + (size_t)(8 * (J + 1) + i) * ostride); }                  \
                 _Pragma("unroll") for (int i = 0; i < 8; i += 2)                                        \
-                    if (live) st_stream4(save + (4 * J + i / 2) * NT, v[8 * J + i], v[8 * J + i + 1]);  \
+                    st_stream4(save + (4 * J + i / 2) * NT, v[8 * J + i], v[8 * J + i + 1]);            \
                 _Pragma("unroll") for (int i = 0; i < 8; ++i) v[8 * J + i] = cmul(v[8 * J + i], CUR[i]); \
             }
             PTY_G2_CHUNK(0, oa, ob) PTY_G2_CHUNK(1, ob, oa) PTY_G2_CHUNK(2, oa, ob) PTY_G2_CHUNK(3, ob, oa)
@@ -285,7 +317,7 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
 #pragma unroll
             for (int r = 0; r < 32; ++r) {
                 v[r] = cmul(v[r], cmul(my, c.Mx[c.kx(o, r)]));
-                if (HAT && live) st_stream2(hat + r * NT, v[r]);
+                if (HAT) st_stream2(hat + r * NT, v[r]);
             }
             g2_radix4<+1>(c, o, v);
             g2_st_slots(c, o, v);
@@ -305,18 +337,16 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
 #pragma unroll
         for (int r = 0; r < 32; r += 2) {
             const float2 p0 = cscale(v[r], 1.0f / N), p1 = cscale(v[r + 1], 1.0f / N);
-            if (live) {
-                st_stream2(Psi + r * NT, p0);
-                st_stream2(Psi + (r + 1) * NT, p1);
-                red_add2(Ib + (r >> 1) * NT + 128 * o + c.c, make_float2(p0.x * p0.x + p0.y * p0.y, p1.x * p1.x + p1.y * p1.y));
-            }
+            st_stream2(Psi + r * NT, p0);
+            st_stream2(Psi + (r + 1) * NT, p1);
+            red_add2(Ib + (r >> 1) * NT + 128 * o + c.c, make_float2(p0.x * p0.x + p0.y * p0.y, p1.x * p1.x + p1.y * p1.y));
         }
     }
     if (c.G == 0) c.acquireX();      // consume group 1's last release
 }
 
 // ------------------------------------------------------------------------------ adjoint (a7-a13)
-template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, bool live) {
+template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, int slot, float scl) {
     constexpr int N = 128, NT = F128::NT;
     int b, m;
     size_t obj_off;
@@ -325,7 +355,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
     setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
     c.grp_sync();
     const size_t NN = (size_t)N * N;
-    const size_t bm = (size_t)item;
+    const size_t bm = (size_t)slot;
     float2 v[32];
     NoBg bg;
     {   // a7, a8 (K): g_Psi = w Psi, inverse x radix-4 -> role blocks
@@ -335,7 +365,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
             const float2* Psi = A.ws_Psi + bm * NN + 128 * o + c.c;
             const float* Wt = A.seed_w + (size_t)b * NN + 128 * o + c.c;
 #pragma unroll
-            for (int r = 0; r < 32; ++r) v[r] = cscale(ld_stream2(Psi + r * NT), ldg1(Wt + r * NT));
+            for (int r = 0; r < 32; ++r) v[r] = cscale(ld_stream2(Psi + r * NT), ldg1(Wt + r * NT) * scl);
             g2_radix4<+1>(c, o, v);
             g2_st_slots(c, o, v);
         }
@@ -348,8 +378,25 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
         first = false;
         // a9, a10 (R): g = fft32^-1; g_object patch += conj(psi_{s-1}) g; g <- conj(O_b[s]) g; forward y first stage.
         // Park-then-stream: both roles' g goes back to its TMEM block first, which frees the 64 wave registers;
-        // the pointwise step then streams over the 16 chunks of 4 rows (two roles x 8) with the saved wave
-        // (HBM stream) and the object rows five chunks ahead in registers and g one chunk ahead from TMEM.
+        // the pointwise step then streams over the 16 chunks of 4 rows (two roles x 8) with the saved wave (HBM
+        // stream) and the object rows D chunks ahead in registers and g one chunk ahead from TMEM.  The first D
+        // chunks of the saved wave are requested BEFORE the two inverse fft32 of the park phase (PTY_G2_EARLY):
+        // that arithmetic covers the HBM latency of the stream's start.
+        constexpr int D = PTY_G2_D;
+        const float4* psi0 = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 256 * c.gg + c.c;
+        float4 pb[D][2];
+#define PTY_G2_ISSUE_PSI(J)                                                                               \
+        {                                                                                                 \
+            const float4* pp_ = psi0 + 128 * ((J) >> 3) + (size_t)(2 * ((J) & 7)) * NT;                   \
+            pb[(J) % D][0] = g2_ld_psi(pp_);                                                              \
+            pb[(J) % D][1] = g2_ld_psi(pp_ + NT);                                                         \
+        }
+#if PTY_G2_EARLY
+        PTY_G2_ISSUE_PSI(0) PTY_G2_ISSUE_PSI(1) PTY_G2_ISSUE_PSI(2)
+        if (D > 3) PTY_G2_ISSUE_PSI(3)
+        if (D > 4) PTY_G2_ISSUE_PSI(4)
+        if (D > 5) PTY_G2_ISSUE_PSI(5)
+#endif
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
             const int o = 2 * c.gg + h;
@@ -359,23 +406,22 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
         }
         tmem_wait_st();
         {
-            constexpr int D = PTY_G2_D;
             const size_t ostride = (size_t)4 * A.W;
             const float2* obj0 = A.object + obj_off + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
             float2* gobj0 = A.g_object + obj_off + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
-            const float4* psi0 = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 256 * c.gg + c.c;
             const unsigned tb0 = c.blk(2 * c.gg);
-            float4 pb[D][2];
             float2 ob[D][4];
             float2 gb[2][4];
-#define PTY_G2_ISSUE(J)                                                                                   \
+#define PTY_G2_ISSUE_OBJ(J)                                                                               \
             {                                                                                             \
-                const float4* pp_ = psi0 + 128 * ((J) >> 3) + (size_t)(2 * ((J) & 7)) * NT;               \
-                pb[(J) % D][0] = ld_stream4_pinned(pp_);                                                  \
-                pb[(J) % D][1] = ld_stream4_pinned(pp_ + NT);                                             \
                 const float2* oo_ = obj0 + (size_t)((J) >> 3) * A.W + (size_t)(4 * ((J) & 7)) * ostride;  \
-                _Pragma("unroll") for (int i = 0; i < 4; ++i) ob[(J) % D][i] = ldg2_pinned(oo_ + (size_t)i * ostride); \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i) ob[(J) % D][i] = g2_ld_obj(oo_ + (size_t)i * ostride); \
             }
+#if PTY_G2_EARLY
+#define PTY_G2_ISSUE(J) PTY_G2_ISSUE_OBJ(J)
+#else
+#define PTY_G2_ISSUE(J) PTY_G2_ISSUE_PSI(J) PTY_G2_ISSUE_OBJ(J)
+#endif
 #define PTY_G2_STEP(J)                                                                                    \
             {                                                                                             \
                 tmem_wait_ld();                                                                           \
@@ -385,11 +431,11 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
                     const float4 q_ = pb[(J) % D][i >> 1];                                                \
                     const float2 ps = (i & 1) ? make_float2(q_.z, q_.w) : make_float2(q_.x, q_.y);        \
                     const float2 g_ = gb[(J) & 1][i];                                                     \
-                    if (live) red_add2(go_ + (size_t)i * ostride, cmulc(ps, g_));                         \
+                    g2_red_obj(go_ + (size_t)i * ostride, cmulc(ps, g_));                                 \
                     gb[(J) & 1][i] = cmulc(ob[(J) % D][i], g_);                                           \
                 }                                                                                         \
                 tmem_st4(tb0 + 64u * ((J) >> 3) + 8u * ((J) & 7), gb[(J) & 1]);                           \
-                if ((J) + D < 16) PTY_G2_ISSUE((J) + D)                                                   \
+                if ((J) + D < 16) { PTY_G2_ISSUE_PSI((J) + D) PTY_G2_ISSUE_OBJ((J) + D) }                 \
             }
             PTY_G2_ISSUE(0) PTY_G2_ISSUE(1) PTY_G2_ISSUE(2)
             if (D > 3) PTY_G2_ISSUE(3)
@@ -401,6 +447,8 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
             PTY_G2_STEP(12) PTY_G2_STEP(13) PTY_G2_STEP(14) PTY_G2_STEP(15)
 #undef PTY_G2_STEP
 #undef PTY_G2_ISSUE
+#undef PTY_G2_ISSUE_OBJ
+#undef PTY_G2_ISSUE_PSI
         }
         tmem_wait_st();
 #pragma unroll 1
@@ -456,7 +504,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
                 const int kx = c.kx(o, r);
                 const float2 gg = v[r];
                 const float2 e = cmul(ey, c.Ex[kx]);                     // E / N
-                if (live) red_add2(GP + r * NT, cmulc(e, gg));
+                red_add2(GP + r * NT, cmulc(e, gg));
                 const float2 ep = cmul(e, ldg2(Ph + r * NT));
                 const float t = gg.x * ep.y - gg.y * ep.x;               // Im(conj(g^_0) E P^)
                 accy += kyf * t;
@@ -472,7 +520,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
         g2_accumulate(c, 4, acc_k2);
     }
     c.grp_sync();
-    if (c.t == 0 && live) {
+    if (c.t == 0) {
         const float two_pi = 6.283185307179586f;
         if (A.g_pos) {
             red_add(A.g_pos + 2 * b, two_pi * c.red[0]);

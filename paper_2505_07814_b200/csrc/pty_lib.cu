@@ -94,7 +94,10 @@ template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_
     const int n = A.B * A.MT;
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         const int item = it + c.G;
-        fwd_body_g2<HAT>(A, c, min(item, n - 1), item < n);
+#ifdef PTY_ABL_ONEGROUP
+        if (c.G == 1) break;
+#endif
+        fwd_body_g2<HAT>(A, c, min(item, n - 1), item, item < n ? 1.f : 0.f);   // item == n: the ghost (slot n)
         c.grp_sync();            // the next body rewrites the group's tables and reduction slots
     }
     release_g2(smem);
@@ -105,8 +108,10 @@ template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_
     const int n = A.B * A.MT;
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         int item = it + c.G;
-        asm volatile("" : "+r"(item));           // keep per-item address arithmetic inside the body (register pressure)
-        bwd_body_g2<HAT>(A, c, min(item, n - 1), item < n);
+#ifdef PTY_ABL_ONEGROUP
+        if (c.G == 1) break;
+#endif
+        bwd_body_g2<HAT>(A, c, min(item, n - 1), item, item < n ? 1.f : 0.f);
         c.grp_sync();
     }
     release_g2(smem);
@@ -316,9 +321,10 @@ Layout make_layout(const pty_dims& d) {
     L.probe_hat = take(M * NN * 8);
     L.prop = take(2 * (size_t)d.N * 8);
     L.I = take(B * NN * 4);
-    L.ws_psi = take(B * MT * Nz * NN * 8);
-    L.ws_Psi = take(B * MT * NN * 8);
-    L.ws_hat = take(save_hat_of(d) ? B * MT * (Nz - 1) * NN * 8 : 0);
+    // + 1: the spare slot of the N = 128 kernels' ghost item (odd item counts)
+    L.ws_psi = take((B * MT + 1) * Nz * NN * 8);
+    L.ws_Psi = take((B * MT + 1) * NN * 8);
+    L.ws_hat = take(save_hat_of(d) ? (B * MT + 1) * (Nz - 1) * NN * 8 : 0);
     L.GP_hat = take(M * NN * 8);
     L.dsum = take(B * 4 * 4);
     L.seed_w = take(B * NN * 4);
