@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpty.so")
 BENCH_LIB = os.path.join(HERE, "libpty_benchutil.so")
-HEADERS = ["pty_port.cuh", "pty_fft.cuh", "pty_kernels.cuh", "pty_fft128.cuh", "pty_kernels128.cuh",
+HEADERS = ["pty_port.cuh", "pty_pointwise.cuh", "pty_fft.cuh", "pty_kernels.cuh", "pty_fft128.cuh", "pty_kernels128.cuh",
            "pty_kernels128g2.cuh", os.path.join("..", "..", "include", "pty.h")]
 TARGETS = {LIB: (["pty_lib.cu"], HEADERS), BENCH_LIB: (["pty_bench_util.cu"], [])}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -53,6 +53,13 @@ PTY_DEV float2 g2_ld_obj(const float2* p) {
 #endif
 }
 
+PTY_DEV void g2_st_psi(float4* p, float2 a, float2 b) {
+#ifdef PTY_ABL_PSI
+    if (a.x == 1.2345e-30f)
+#endif
+    st_stream4(p, a, b);
+}
+
 struct G2Smem {
     static constexpr size_t xch_bytes = F128::xch_bytes;
     // twg[128] | per group: Ey, Ex, My, Mx [128 each] float2, red[64] float | TMEM base
@@ -75,7 +82,7 @@ struct G2 {
         tmem_fence_after_sync();
     }
     PTY_DEV void grp_sync() const { asm volatile("bar.sync %0, 256;" ::"r"(9 + G) : "memory"); }
-#ifdef PTY_ABL_ONEGROUP      // timing ablation: group 1 idles, group 0 owns the transpose buffer
+#if defined(PTY_ABL_ONEGROUP) || defined(PTY_ABL_NOX)   // timing ablations: no hand-over of the transpose buffer
     PTY_DEV void acquireX() const {}
     PTY_DEV void releaseX() const {}
 #else
@@ -287,16 +294,16 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
             const size_t ostride = (size_t)4 * A.W;
             float2 oa[8], ob[8];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) oa[i] = ldg2_pinned(obj + (size_t)i * ostride);
+            for (int i = 0; i < 8; ++i) oa[i] = g2_ld_obj(obj + (size_t)i * ostride);
             g2_ld_own(c, o, v);
             fft32<+1, 0>(v, bg);
             float4* save = reinterpret_cast<float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 128 * o + c.c;
 #define PTY_G2_CHUNK(J, CUR, NXT)                                                                       \
             {                                                                                           \
                 if (J < 3) { _Pragma("unroll") for (int i = 0; i < 8; ++i)                              \
-                    NXT[i] = ldg2_pinned(obj + (size_t)(8 * (J + 1) + i) * ostride); }                  \
+                    NXT[i] = g2_ld_obj(obj + (size_t)(8 * (J + 1) + i) * ostride); }                    \
                 _Pragma("unroll") for (int i = 0; i < 8; i += 2)                                        \
-                    st_stream4(save + (4 * J + i / 2) * NT, v[8 * J + i], v[8 * J + i + 1]);            \
+                    g2_st_psi(save + (4 * J + i / 2) * NT, v[8 * J + i], v[8 * J + i + 1]);             \
                 _Pragma("unroll") for (int i = 0; i < 8; ++i) v[8 * J + i] = cmul(v[8 * J + i], CUR[i]); \
             }
             PTY_G2_CHUNK(0, oa, ob) PTY_G2_CHUNK(1, ob, oa) PTY_G2_CHUNK(2, oa, ob) PTY_G2_CHUNK(3, ob, oa)
@@ -418,9 +425,9 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
                 _Pragma("unroll") for (int i = 0; i < 4; ++i) ob[(J) % D][i] = g2_ld_obj(oo_ + (size_t)i * ostride); \
             }
 #if PTY_G2_EARLY
-#define PTY_G2_ISSUE(J) PTY_G2_ISSUE_OBJ(J)
+#define PTY_G2_ISSUE(J) { PTY_G2_ISSUE_OBJ(J) }
 #else
-#define PTY_G2_ISSUE(J) PTY_G2_ISSUE_PSI(J) PTY_G2_ISSUE_OBJ(J)
+#define PTY_G2_ISSUE(J) { PTY_G2_ISSUE_PSI(J) PTY_G2_ISSUE_OBJ(J) }   // one statement: used under `if (D > n)`
 #endif
 #define PTY_G2_STEP(J)                                                                                    \
             {                                                                                             \
