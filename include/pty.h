@@ -70,6 +70,12 @@ extern "C" {
 #define PTY_FLAG_HOST          4    /* reserve device staging buffers: pty_grad_host           */
 #define PTY_FLAG_AMP_PHASE     8    /* reserve the composed object, its gradient and the patch
                                        coverage map: pty_*_ap (amplitude / phase object)       */
+#define PTY_FLAG_TMA_OBJECT   16    /* N = 128, forward kernel: stage the first 12 rows of every role's
+                                       object patch column with TMA (cp.async.bulk.tensor into a shared-
+                                       memory ring) instead of fetching all rows through registers; same
+                                       results.  Needs an even W and a 16-byte aligned `object`, otherwise
+                                       the register path runs.  Off by default: measured slower on c4
+                                                                                  */
 
 /* pty_backward flags */
 #define PTY_BWD_ACCUMULATE     1    /* add into the gradient outputs instead of overwriting    */

@@ -60,11 +60,29 @@ PTY_DEV void g2_st_psi(float4* p, float2 a, float2 b) {
     st_stream4(p, a, b);
 }
 
+// timeline instrumentation (never defined in the product build): lane 0 of every warp of CTA 0 logs (event id, SM clock)
+#ifdef PTY_TRACE
+__device__ long long g_trace[16 * 1024];
+__device__ int g_trace_n[16];
+PTY_DEV void g2_trace(int ev) {
+    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {
+        const int w = threadIdx.x >> 5;
+        const int n = g_trace_n[w];
+        if (n < 1024) { g_trace[w * 1024 + n] = ((long long)ev << 48) | (clock64() & 0xffffffffffffLL); g_trace_n[w] = n + 1; }
+    }
+}
+#else
+PTY_DEV void g2_trace(int) {}
+#endif
+
 struct G2Smem {
     static constexpr size_t xch_bytes = F128::xch_bytes;
     // twg[128] | per group: Ey, Ex, My, Mx [128 each] float2, red[64] float | TMEM base
     static constexpr size_t group_bytes = 4 * 128 * sizeof(float2) + 64 * sizeof(float);
-    static constexpr size_t bytes = xch_bytes + 128 * sizeof(float2) + 2 * group_bytes + 16;
+#ifndef PTY_ABL_SMEM_PAD
+#define PTY_ABL_SMEM_PAD 0      // timing ablation: extra dynamic shared memory (shrinks L1)
+#endif
+    static constexpr size_t bytes = xch_bytes + 128 * sizeof(float2) + 2 * group_bytes + 16 + PTY_ABL_SMEM_PAD;
 };
 
 struct G2 {
@@ -125,6 +143,75 @@ PTY_DEV void release_g2(unsigned char* smem) {
     if ((threadIdx.x >> 5) == 0) tmem_dealloc512(*tbase);
 }
 
+// ------------------------------------------------------------------------------ TMA ring of object rows
+// The crop of PAPER.md:75-81 as a TMA gather: the object [Nobj][Nz][H][W] is one 3-D tensor (x, row % 4, row / 4) of
+// 8-byte elements, so the rows y = 4 i + o that one role of the FFT needs (layout R) are a box {130, 1, R}: a TMA box
+// has to start on a 16-byte boundary of global memory, so it starts at the even column rx & ~1 and is 130 wide (columns
+// past the object's edge are zero-filled and never read).  Each
+// half-group (128 threads = one role at a time) owns S slots of 4 rows; one elected thread issues the boxes of the
+// NEXT role-step (next role, next slice or next item) as soon as the current one has been consumed, so the rows are
+// in shared memory long before the multiply needs them -- no registers in flight, no LSU address arithmetic, no L1.
+// The remaining rows of a role (32 - 4 S) still come through registers (requested before the preceding transform).
+struct G2Ring {
+    static constexpr int S = 3, ROWS = 4, COLS = 130;
+    static constexpr unsigned slot_bytes = ROWS * COLS * sizeof(float2);            // what one box transfers
+    static constexpr unsigned slot_pitch = (slot_bytes + 127) / 128 * 128;          // slots are 128-byte aligned
+    static constexpr int slot_elems = slot_pitch / sizeof(float2);
+    static constexpr size_t offset = (G2Smem::bytes + 1023) / 1024 * 1024;
+    static constexpr size_t bytes = offset + 4 * S * slot_pitch + 4 * 2 * S * sizeof(unsigned long long);
+    float2* slots;                        // this half-group's S slots, [S][ROWS][COLS] (pitch slot_elems)
+    unsigned long long *full, *empty;     // [S] each
+    const CUtensorMap* tm;
+    unsigned cpar, ppar;                  // parity of the consumer's next full wait / of the generation the producer fills next
+    bool producer;
+};
+
+PTY_DEV G2Ring make_g2_ring(unsigned char* smem, const G2& c, const CUtensorMap* tm) {
+    G2Ring r;
+    const int hg = 2 * c.G + c.gg;        // half-group
+    r.slots = reinterpret_cast<float2*>(smem + G2Ring::offset + (size_t)hg * G2Ring::S * G2Ring::slot_pitch);
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem + G2Ring::offset + 4 * G2Ring::S * G2Ring::slot_pitch);
+    r.full = bars + hg * 2 * G2Ring::S;
+    r.empty = r.full + G2Ring::S;
+    r.tm = tm;
+    r.cpar = 0; r.ppar = 0;
+    r.producer = (c.t & 127) == 0;
+    if (r.producer) {
+#pragma unroll
+        for (int k = 0; k < G2Ring::S; ++k) { mbar_init(r.full + k, 1); mbar_init(r.empty + k, 4); }
+        mbar_init_fence();
+        tma_prefetch_desc(tm);
+    }
+    __syncthreads();
+    return r;
+}
+
+// rows (row0 + 4 i), i < 4 S, columns [rx & ~1, +130) -> the half-group's slots (producer thread only)
+PTY_DEV void g2_ring_fill(G2Ring& r, int rx, int row0) {
+#pragma unroll
+    for (int k = 0; k < G2Ring::S; ++k) {
+        mbar_wait(r.empty + k, r.ppar ^ 1u);
+        mbar_expect_tx(r.full + k, G2Ring::slot_bytes);
+        tma_load_3d(r.slots + k * G2Ring::slot_elems, r.tm, rx & ~1, row0 & 3, (row0 >> 2) + G2Ring::ROWS * k, r.full + k);
+    }
+    r.ppar ^= 1u;
+}
+
+// crop origin of position b (the same arithmetic as setup_factors: F1 with the clamp of reading R22)
+PTY_DEV void g2_crop_origin(const KArgs& A, int b, int& ry, int& rx) {
+    const double py = (double)A.positions[2 * b], px = (double)A.positions[2 * b + 1];
+    const int iy = (int)floor(py + 0.5), ix = (int)floor(px + 0.5);
+    ry = min(max(iy, 0), A.H - 128); rx = min(max(ix, 0), A.W - 128);
+}
+// first object row of (item, slice 0, role o) in the 3-D view, and its first column
+PTY_DEV void g2_item_rows(const KArgs& A, int item, int o, int& row0, int& rx) {
+    int b, m, ry;
+    size_t obj_off;
+    decode_item(A, item, b, m, obj_off);
+    g2_crop_origin(A, b, ry, rx);
+    row0 = (int)(obj_off / (size_t)A.W) + ry + o;
+}
+
 // ------------------------------------------------------------------------------ radix-4 stage with twiddles
 // DIR < 0: v[8 q + i] -> twiddle W128^(q (8 o + i)) -> radix-4 over q -> v[8 k2 + i]   (forward)
 // DIR > 0: v[8 k2 + i] -> inverse radix-4 over k2 -> conj twiddle -> v[8 q + i]         (inverse)
@@ -178,8 +265,10 @@ PTY_DEV void g2_st_slots(const G2& c, int o, float2 (&v)[32]) {
 PTY_DEV void g2_inverse_head(const G2& c, float2 (&v)[32], bool first) {
     constexpr int P = F128::P;
     NoBg bg;
+    g2_trace(1);
     c.pair_sync();
     if (!first) c.acquireX();
+    g2_trace(2);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -189,7 +278,9 @@ PTY_DEV void g2_inverse_head(const G2& c, float2 (&v)[32], bool first) {
 #pragma unroll
         for (int n = 0; n < 32; ++n) s[4 * n] = v[n];
     }
+    g2_trace(3);
     c.grp_sync();
+    g2_trace(4);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -201,12 +292,14 @@ PTY_DEV void g2_inverse_head(const G2& c, float2 (&v)[32], bool first) {
             v[16 + i] = s[(i + 64) * P];
             v[24 + i] = s[(i + 96) * P];
         }
-        if (h == 1) c.releaseX();
+        if (h == 1) { c.releaseX(); g2_trace(5); }
         g2_radix4<+1>(c, o, v);
         g2_st_slots(c, o, v);
     }
     tmem_wait_st();
+    g2_trace(6);
     c.pair_sync();
+    g2_trace(7);
 }
 
 // Forward transform after the per-role fft32<-1> + g2_st_own of the caller: role blocks -> y radix-4 -> X ->
@@ -215,8 +308,10 @@ PTY_DEV void g2_forward_tail(const G2& c, float2 (&v)[32]) {
     constexpr int P = F128::P;
     NoBg bg;
     tmem_wait_st();
+    g2_trace(8);
     c.pair_sync();
     c.acquireX();
+    g2_trace(9);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -226,7 +321,9 @@ PTY_DEV void g2_forward_tail(const G2& c, float2 (&v)[32]) {
 #pragma unroll
         for (int r = 0; r < 32; ++r) s[((r & 7) + 32 * (r >> 3)) * P] = v[r];
     }
+    g2_trace(10);
     c.grp_sync();
+    g2_trace(11);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -238,12 +335,14 @@ PTY_DEV void g2_forward_tail(const G2& c, float2 (&v)[32]) {
             v[16 + n2] = s[4 * (16 + n2)];
             v[24 + n2] = s[4 * (24 + n2)];
         }
-        if (h == 1) c.releaseX();
+        if (h == 1) { c.releaseX(); g2_trace(12); }
         fft32<-1, 0>(v, bg);
         g2_st_own(c, o, v);
     }
     tmem_wait_st();
+    g2_trace(13);
     c.pair_sync();
+    g2_trace(14);
 }
 
 PTY_DEV void g2_accumulate(const G2& c, int slot, float v) {
@@ -257,7 +356,10 @@ PTY_DEV void g2_accumulate(const G2& c, int slot, float v) {
 // that every reduction it issues adds zero and no store, reduction or load in these bodies needs a predicate.
 // HAT: keep the propagated spectra (tilt / dz gradients); a compile-time switch so that the common no-tilt kernels
 // carry neither the code nor the registers of that path.
-template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int item, int slot, float scl) {
+// TMA: the first 4 S object rows of every role come from the half-group's TMA ring (`ring`; `next_item` = the item this
+// group runs after this one, -1 if none: its first rows are requested at the end of this body).
+template <bool HAT, bool TMA>
+PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, int slot, float scl, int next_item) {
     constexpr int N = 128, NT = F128::NT;
     int b, m;
     size_t obj_off;
@@ -293,23 +395,82 @@ template <bool HAT> PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, int it
             const float2* obj = A.object + obj_off + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
             const size_t ostride = (size_t)4 * A.W;
             float2 oa[8], ob[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) oa[i] = g2_ld_obj(obj + (size_t)i * ostride);
-            g2_ld_own(c, o, v);
-            fft32<+1, 0>(v, bg);
             float4* save = reinterpret_cast<float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 128 * o + c.c;
+#define PTY_G2_SAVE(J)                                                                                  \
+            { _Pragma("unroll") for (int i = 0; i < 8; i += 2)                                          \
+                g2_st_psi(save + (4 * J + i / 2) * NT, v[8 * J + i], v[8 * J + i + 1]); }
+            if constexpr (TMA) {
+                // rows 0..11 from the ring, 12..19 (oa) and 20..27 (ob) requested now, 28..31 once oa[0..3] are free
+                static_assert(G2Ring::S == 3 && G2Ring::ROWS == 4, "row split of the TMA path");
+#pragma unroll
+                for (int i = 0; i < 8; ++i) oa[i] = g2_ld_obj(obj + (size_t)(12 + i) * ostride);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) ob[i] = g2_ld_obj(obj + (size_t)(20 + i) * ostride);
+                g2_ld_own(c, o, v);
+                fft32<+1, 0>(v, bg);
+                const float2* rs = ring.slots + (rx & 1) + c.c;
+                constexpr int RS = G2Ring::slot_elems, RC = G2Ring::COLS;
+                PTY_G2_SAVE(0)
+                mbar_wait(ring.full + 0, ring.cpar);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[i] = cmul(v[i], rs[i * RC]);
+                mbar_wait(ring.full + 1, ring.cpar);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[4 + i] = cmul(v[4 + i], rs[RS + i * RC]);
+                PTY_G2_SAVE(1)
+                mbar_wait(ring.full + 2, ring.cpar);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[8 + i] = cmul(v[8 + i], rs[2 * RS + i * RC]);
+                ring.cpar ^= 1u;
+                __syncwarp();
+                if (warp_leader()) { mbar_arrive(ring.empty + 0); mbar_arrive(ring.empty + 1); mbar_arrive(ring.empty + 2); }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[12 + i] = cmul(v[12 + i], oa[i]);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) oa[i] = g2_ld_obj(obj + (size_t)(28 + i) * ostride);
+                PTY_G2_SAVE(2)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[16 + i] = cmul(v[16 + i], oa[4 + i]);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[20 + i] = cmul(v[20 + i], ob[i]);
+                PTY_G2_SAVE(3)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[24 + i] = cmul(v[24 + i], ob[4 + i]);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) v[28 + i] = cmul(v[28 + i], oa[i]);
+            } else {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) oa[i] = g2_ld_obj(obj + (size_t)i * ostride);
+                g2_ld_own(c, o, v);
+                fft32<+1, 0>(v, bg);
 #define PTY_G2_CHUNK(J, CUR, NXT)                                                                       \
-            {                                                                                           \
-                if (J < 3) { _Pragma("unroll") for (int i = 0; i < 8; ++i)                              \
-                    NXT[i] = g2_ld_obj(obj + (size_t)(8 * (J + 1) + i) * ostride); }                    \
-                _Pragma("unroll") for (int i = 0; i < 8; i += 2)                                        \
-                    g2_st_psi(save + (4 * J + i / 2) * NT, v[8 * J + i], v[8 * J + i + 1]);             \
-                _Pragma("unroll") for (int i = 0; i < 8; ++i) v[8 * J + i] = cmul(v[8 * J + i], CUR[i]); \
-            }
-            PTY_G2_CHUNK(0, oa, ob) PTY_G2_CHUNK(1, ob, oa) PTY_G2_CHUNK(2, oa, ob) PTY_G2_CHUNK(3, ob, oa)
+                {                                                                                       \
+                    if (J < 3) { _Pragma("unroll") for (int i = 0; i < 8; ++i)                          \
+                        NXT[i] = g2_ld_obj(obj + (size_t)(8 * (J + 1) + i) * ostride); }                \
+                    PTY_G2_SAVE(J)                                                                      \
+                    _Pragma("unroll") for (int i = 0; i < 8; ++i) v[8 * J + i] = cmul(v[8 * J + i], CUR[i]); \
+                }
+                PTY_G2_CHUNK(0, oa, ob) PTY_G2_CHUNK(1, ob, oa) PTY_G2_CHUNK(2, oa, ob) PTY_G2_CHUNK(3, ob, oa)
 #undef PTY_G2_CHUNK
+            }
+#undef PTY_G2_SAVE
             fft32<-1, 0>(v, bg);
             g2_st_own(c, o, v);
+            if constexpr (TMA) {
+                // the ring's slots are free again (every warp of the half-group has arrived or will shortly): request the
+                // rows of the next role-step -- the other role of this slice, the first role of the next slice, or of the
+                // next item
+                if (ring.producer) {
+                    const int row_now = (int)(obj_off / (size_t)A.W) + s * A.H + ry + o;
+                    if (h == 0) g2_ring_fill(ring, rx, row_now + 1);
+                    else if (s + 1 < A.Nz) g2_ring_fill(ring, rx, row_now - 1 + A.H);
+                    else if (next_item >= 0) {
+                        int row0, rxn;
+                        g2_item_rows(A, next_item, 2 * c.gg, row0, rxn);
+                        g2_ring_fill(ring, rxn, row0);
+                    }
+                }
+            }
         }
         g2_forward_tail(c, v);
         if (s == A.Nz - 1) break;

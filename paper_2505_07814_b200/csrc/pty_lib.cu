@@ -86,18 +86,32 @@ __device__ __forceinline__ void release_cta128(unsigned char* smem) {
 }
 
 // N = 128, two items per CTA (pty_kernels128g2.cuh): group G of CTA x owns item 2 x + G
-template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A) {
-    extern __shared__ __align__(16) unsigned char smem[];
+// TMA: object rows staged by TMA (tmObj = the 3-D view of the object, make_object_map); false = register path only
+// (odd W or an object pointer that is not 16-byte aligned, for which no tensor map exists).
+template <bool HAT, bool TMA>
+__global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A, const __grid_constant__ CUtensorMap tmObj) {
+    extern __shared__ __align__(1024) unsigned char smem[];
     const G2 c = make_g2(smem);
     // persistent CTAs: TMEM allocation and the twiddle table once per SM; CTA x takes the item pairs x, x + grid, ...
     // (both groups run the same number of bodies: the hand-over of the transpose buffer is balanced per body)
     const int n = A.B * A.MT;
+    G2Ring ring{};
+    if constexpr (TMA) {
+        ring = make_g2_ring(smem, c, &tmObj);
+        if (ring.producer && 2 * (int)blockIdx.x < n) {      // the first role-step of this group's first item
+            int row0, rx;
+            g2_item_rows(A, min(2 * (int)blockIdx.x + c.G, n - 1), 2 * c.gg, row0, rx);
+            g2_ring_fill(ring, rx, row0);
+        }
+    }
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         const int item = it + c.G;
 #ifdef PTY_ABL_ONEGROUP
         if (c.G == 1) break;
 #endif
-        fwd_body_g2<HAT>(A, c, min(item, n - 1), item, item < n ? 1.f : 0.f);   // item == n: the ghost (slot n)
+        const int itn = it + 2 * (int)gridDim.x;
+        fwd_body_g2<HAT, TMA>(A, c, ring, min(item, n - 1), item, item < n ? 1.f : 0.f,   // item == n: the ghost (slot n)
+                              itn < n ? min(itn + c.G, n - 1) : -1);
         c.grp_sync();            // the next body rewrites the group's tables and reduction slots
     }
     release_g2(smem);
@@ -372,6 +386,8 @@ struct pty_plan {
     const void *f_object, *f_probe, *f_positions, *f_tilt, *f_meas;
     int32_t f_B;
 
+    CUtensorMap tm_obj;          // TMA view of the object last seen by a forward / adjoint launch (object_map)
+    const void* tm_obj_ptr;
     pty_loss loss_cfg;           // pty_set_loss; mode 0 = plain amplitude sum
     bool sparse_ready;           // the AP forward has put L_sparse into the statistics of this call
     // optional kernel timing (pty_profile)
@@ -479,15 +495,57 @@ template <class SH> cudaError_t launch_fwd_sh(pty_plan* p, const KArgs& A, cudaS
 template <class SH> cudaError_t launch_bwd_sh(pty_plan* p, const KArgs& A, cudaStream_t st) {
     return launch(p, pty_bwd_kernel<SH>, A.B * A.MT * SH::CL, SH::NT, ShapeInfo<SH>::smem_bytes, SH::CL, st, A);
 }
+// ---- the object as a TMA tensor (G2Ring): 3-D view (x, row % 4, row / 4) of 8-byte elements, box {130, 1, 4}.
+// cuTensorMapEncodeTiled comes from the driver through the runtime (no link against libcuda).  The map is cached per
+// object pointer; TMA needs a 16-byte aligned base and row pitch, otherwise the register path runs.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            f = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(f);
+    }();
+    return fn;
+}
+// true when `object` can be read through TMA; fills p->tm_obj (cached)
+bool object_map(pty_plan* p, const void* object) {
+    const pty_dims& d = p->d;
+    if (d.N != 128 || (d.W & 1) || (reinterpret_cast<uintptr_t>(object) & 15) || !(p->d.flags & PTY_FLAG_TMA_OBJECT)) return false;
+    if (p->tm_obj_ptr == object) return true;
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return false;
+    const cuuint64_t rows = (cuuint64_t)p->n_obj() * d.Nz * d.H;
+    const cuuint64_t dims[3] = {(cuuint64_t)d.W, 4, (rows + 3) / 4};
+    const cuuint64_t strides[2] = {(cuuint64_t)d.W * 8, (cuuint64_t)d.W * 32};     // bytes, dims 1 and 2
+    const cuuint32_t box[3] = {(cuuint32_t)G2Ring::COLS, 1, (cuuint32_t)G2Ring::ROWS};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (enc(&p->tm_obj, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void*>(object), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    p->tm_obj_ptr = object;
+    return true;
+}
+
 int g2_grid(const pty_plan* p, const KArgs& A) {      // one persistent CTA per SM, or fewer when there is less work
     const int pairs = (A.B * A.MT + 1) / 2;
     return pairs < p->num_sms ? pairs : p->num_sms;
 }
 cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 0, st);
-    if (p->d.N == 128)
-        return A.save_hat ? launch(p, pty_fwd128g2_kernel<true>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A)
-                          : launch(p, pty_fwd128g2_kernel<false>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A);
+    if (p->d.N == 128) {
+        const int grid = g2_grid(p, A);
+        if (object_map(p, A.object))
+            return A.save_hat ? launch(p, pty_fwd128g2_kernel<true, true>, grid, F128::NT, G2Ring::bytes, 1, st, A, p->tm_obj)
+                              : launch(p, pty_fwd128g2_kernel<false, true>, grid, F128::NT, G2Ring::bytes, 1, st, A, p->tm_obj);
+        return A.save_hat ? launch(p, pty_fwd128g2_kernel<true, false>, grid, F128::NT, G2Smem::bytes, 1, st, A, p->tm_obj)
+                          : launch(p, pty_fwd128g2_kernel<false, false>, grid, F128::NT, G2Smem::bytes, 1, st, A, p->tm_obj);
+    }
     return p->d.N == 64 ? launch_fwd_sh<Shape<64>>(p, A, st) : launch_fwd_sh<Shape<256>>(p, A, st);
 }
 cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
@@ -686,7 +744,7 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
     pty_plan* p = new (std::nothrow) pty_plan();
     if (!p) return fail(nullptr, PTY_ERR_INVALID_ARG, "out of host memory");
     p->d = *dims; p->L = L; p->ws = static_cast<unsigned char*>(workspace); p->device = device;
-    p->last_stream = nullptr; p->launches = 0; p->fwd_valid = false; p->profiling = false;
+    p->last_stream = nullptr; p->launches = 0; p->fwd_valid = false; p->profiling = false; p->tm_obj_ptr = nullptr;
     p->loss_cfg = pty_loss{0, 1.f, 0.f, 0.f, 0.f, 1e-6f}; p->sparse_ready = false;
     int prev_device = -1;
     cudaError_t e = cudaGetDevice(&prev_device);
@@ -701,9 +759,13 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
     if (e == cudaSuccess && dims->N == 64) e = set_smem_attrs<Shape<64>>();
     if (e == cudaSuccess && dims->N == 256) e = set_smem_attrs<Shape<256>>();
     if (e == cudaSuccess && dims->N == 128) {
-        e = cudaFuncSetAttribute(pty_fwd128g2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+        e = cudaFuncSetAttribute(pty_fwd128g2_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(pty_fwd128g2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+            e = cudaFuncSetAttribute(pty_fwd128g2_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_fwd128g2_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Ring::bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_fwd128g2_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Ring::bytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_bwd128g2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)
@@ -1111,4 +1173,15 @@ int64_t pty_launch_count(const pty_plan* plan) { return plan ? plan->launches : 
 
 const char* pty_last_error(const pty_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
 
+#ifdef PTY_TRACE
+// timeline instrumentation (debug builds only): copies the trace of CTA 0 out and resets it
+int pty_trace_read(long long* host_events, int* host_counts) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(host_events, pty::g_trace, sizeof(long long) * 16 * 1024);
+    cudaMemcpyFromSymbol(host_counts, pty::g_trace_n, sizeof(int) * 16);
+    int zero[16] = {0};
+    cudaMemcpyToSymbol(pty::g_trace_n, zero, sizeof(zero));
+    return 0;
+}
+#endif
 }  // extern "C"

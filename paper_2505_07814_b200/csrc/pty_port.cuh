@@ -2,6 +2,7 @@
 // into global memory, streaming loads/stores, fast math), sm_100a only.
 #pragma once
 #define PTY_PORT_INCLUDED
+#include <cuda.h>           // CUtensorMap (type only: the driver entry point is fetched at run time)
 #include <cuda_runtime.h>
 #include <cooperative_groups.h>
 
@@ -104,6 +105,51 @@ PTY_DEV float4 ld_stream4_pinned(const float4* p) {
     return v;
 }
 PTY_DEV void st_stream4(float4* p, float2 a, float2 b) { __stcs(p, make_float4(a.x, a.y, b.x, b.y)); }
+
+// cache warming without a destination register
+PTY_DEV void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+PTY_DEV void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// bulk prefetch of a contiguous range into L2 (one thread, no registers, no L1): bytes % 16 == 0, 16-byte aligned
+PTY_DEV void prefetch_l2_bulk(const void* p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+// ---- mbarrier + TMA (cp.async.bulk.tensor): tiles of a global tensor land in shared memory without passing through
+// registers or L1; one elected thread issues, the consumers wait on the slot's "full" barrier and hand the slot back
+// through its "empty" barrier (one arrival per consumer warp).
+PTY_DEV unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+PTY_DEV void mbar_init(unsigned long long* b, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+PTY_DEV void mbar_init_fence() {      // make the initialised barriers visible to the async proxy
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+PTY_DEV void mbar_expect_tx(unsigned long long* b, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+PTY_DEV void mbar_arrive(unsigned long long* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+PTY_DEV void mbar_wait(unsigned long long* b, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "PTY_MBAR_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra PTY_MBAR_DONE_%=;\n\t"
+        "bra PTY_MBAR_WAIT_%=;\n\t"
+        "PTY_MBAR_DONE_%=:\n\t}" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+// box of a 3-D tensor map -> shared memory (dst 128-byte aligned); completion counted in bytes on `bar`
+PTY_DEV void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst)), "l"(reinterpret_cast<unsigned long long>(tm)), "r"(c0), "r"(c1), "r"(c2),
+                   "r"(smem_u32(bar)) : "memory");
+}
+PTY_DEV void tma_prefetch_desc(const CUtensorMap* tm) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<unsigned long long>(tm)) : "memory");
+}
 
 PTY_DEV void sincospi_f(float x, float* s, float* c) { sincospif(x, s, c); }
 PTY_DEV float rsqrt_f(float x) { return rsqrtf(x); }

@@ -299,3 +299,47 @@ def test_forward_backward_can_be_captured_in_a_cuda_graph(pty):
     assert rel_l2(g_obj.cpu().numpy(), ref["g_object"]) <= GRAD_RTOL
     assert rel_l2(g_obj.cpu().numpy(), eager[1].cpu().numpy()) <= 1e-5
     assert plan.status()[0] == 0
+
+
+# ----------------------------------------------------------------------------- TMA staging of the object patch
+@pytest.mark.parametrize("c,B,over", [(3, 7, dict(Nz=3, M=3)), (2, 9, {}), (4, 3, {})])
+def test_tma_staged_object_rows_match_the_oracle(pty, c, B, over):
+    """PTY_FLAG_TMA_OBJECT: the first 12 rows of every role's patch column reach the forward kernel through a TMA ring
+    (the crop of PAPER.md:75-81 as cp.async.bulk.tensor boxes).  Same results as the register path: loss, intensities
+    and every gradient against the oracle; crop origins of both parities (a TMA box starts on an even column), an odd
+    item count (ghost item: c3 with M = 3, B = 7) and more than one item per group."""
+    case = small_case(c, B, **over)
+    cfg = case["cfg"]
+    assert {int(np.floor(p[1] + 0.5)) & 1 for p in case["positions"]} == {0, 1}
+    from test_gpu_parity import check_against_oracle, run_gpu
+    ref = oracle.grad_batch(case["object"], case["probe"], case["positions"], case["tilt"], case["meas"], geom_of(cfg))
+    res = run_gpu(pty, case, flags=pty.PTY_FLAG_TMA_OBJECT)
+    _, _, I_ref = oracle.forward_loss_batch(case["object"], case["probe"], case["positions"], case["tilt"], case["meas"],
+                                            geom_of(cfg))
+    assert np.max(np.abs(res["intensity"] - I_ref)) <= 1e-4 * I_ref.max()
+    check_against_oracle(res, ref, case)
+    plain = run_gpu(pty, case)
+    assert rel_l2(res["g_object"], plain["g_object"]) <= 1e-5
+
+
+def test_tma_flag_falls_back_when_the_object_cannot_be_mapped(pty):
+    """An object whose base address is only 8-byte aligned (a view starting at an odd element) cannot be a TMA tensor:
+    the flag is then ignored and the register path runs -- same answer, no error."""
+    case = small_case(3, 4, Nz=2, M=2)
+    cfg = case["cfg"]
+    from test_gpu_parity import check_against_oracle, run_gpu
+    ref = oracle.grad_batch(case["object"], case["probe"], case["positions"], case["tilt"], case["meas"], geom_of(cfg))
+    B = len(case["positions"])
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, flags=pty.PTY_FLAG_TMA_OBJECT)
+    flat = torch.zeros(case["object"].size + 1, dtype=torch.complex64, device="cuda")
+    obj = flat[1:].view(case["object"].shape)
+    obj.copy_(dev(case["object"]))
+    assert obj.data_ptr() % 16 == 8
+    probe, pos, meas = dev(case["probe"]), dev(case["positions"]), dev(case["meas"])
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    g_obj, g_probe, g_pos = torch.zeros_like(dev(case["object"])), torch.zeros_like(probe), torch.zeros(B, 2, device="cuda")
+    plan.forward_loss(obj, probe, pos, None, meas, loss)
+    plan.backward(obj, probe, pos, None, meas, g_obj, g_probe, g_pos, flags=pty.PTY_BWD_REUSE_FORWARD)
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * ref["loss"]
+    assert rel_l2(g_obj.cpu().numpy(), ref["g_object"]) <= GRAD_RTOL
+    assert plan.status()[0] == 0
