@@ -73,6 +73,102 @@ template <int J, int DIR> PTY_DEV float2 mul_w32(float2 a) {
     else return mul_cs<DIR>(a, c, s);
 }
 
+// ---- FMA-form twiddles.  w u = gamma (alpha u + beta (i u)) with |alpha|, |beta| <= 1 and one of them 1: the inner
+// bracket u' is ONE packed FMA, and the real scale gamma is carried as "pending" into the add/sub pair that consumes
+// the value (y +- gamma u' = two packed FMAs instead of two packed adds): 3 packed instructions per twiddled
+// butterfly input instead of 4, and no extra rounding step.  All constants are compile-time.
+#ifndef PTY_FMA_FORM
+#define PTY_FMA_FORM 1
+#endif
+PTY_DEV constexpr double cd32(int j) {
+    constexpr double t[9] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
+                             0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
+                             0.19509032201612826785, 0.0};
+    j &= 31;
+    return j <= 8 ? t[j] : j <= 16 ? -t[16 - j] : j <= 24 ? -t[j - 16] : t[32 - j];
+}
+PTY_DEV constexpr double dabs_(double x) { return x < 0 ? -x : x; }
+// w = exp(i DIR 2 pi J / 32)
+template <int J, int DIR> struct TwC {
+    static constexpr int Jm = ((J % 32) + 32) % 32;
+    static constexpr double C = cd32(Jm), S = DIR * cd32(Jm - 8);
+    static constexpr bool trivial = (Jm % 8 == 0);
+    static constexpr bool caseA = dabs_(C) >= dabs_(S);
+    static constexpr float gamma = trivial ? 1.0f : (caseA ? (float)C : (float)S);
+    static constexpr float T = trivial ? 0.0f : (caseA ? (float)(S / C) : (float)(C / S));
+    // u' with w u = gamma u'
+    static PTY_DEV float2 prep(float2 u) {
+        if constexpr (Jm == 0) return u;
+        else if constexpr (Jm == 8) return mul_qi<DIR>(u);
+        else if constexpr (Jm == 16) return make_float2(-u.x, -u.y);
+        else if constexpr (Jm == 24) return mul_qi<-DIR>(u);
+        else if constexpr (caseA) return __ffma2_rn(make_float2(u.y, u.x), make_float2(-T, T), u);
+        else return __ffma2_rn(u, make_float2(T, T), make_float2(-u.y, u.x));
+    }
+};
+// y + g x, g a compile-time constant at every call site
+PTY_DEV float2 axpy_c(float g, float2 x, float2 y) {
+    if (g == 1.0f) return cadd(y, x);
+    if (g == -1.0f) return csub(y, x);
+    return __ffma2_rn(make_float2(g, g), x, y);
+}
+
+// 8-point DFT over n2 of the values W32^(K1 n2) u[n2] (the twiddles are NOT yet applied to u), natural order out.
+template <int K1, int DIR> PTY_DEV void fft8_pend(float2 (&w)[8]) {
+    using T1 = TwC<K1 * 1, DIR>; using T2 = TwC<K1 * 2, DIR>; using T3 = TwC<K1 * 3, DIR>; using T4 = TwC<K1 * 4, DIR>;
+    using T5 = TwC<K1 * 5, DIR>; using T6 = TwC<K1 * 6, DIR>; using T7 = TwC<K1 * 7, DIR>;
+    constexpr float g1 = T1::gamma, g2 = T2::gamma, g3 = T3::gamma, g4 = T4::gamma, g5 = T5::gamma, g6 = T6::gamma,
+                    g7 = T7::gamma;
+    constexpr float h = 0.70710678118654752440f;
+    const float2 p1 = T1::prep(w[1]), p2 = T2::prep(w[2]), p3 = T3::prep(w[3]), p4 = T4::prep(w[4]),
+                 p5 = T5::prep(w[5]), p6 = T6::prep(w[6]), p7 = T7::prep(w[7]);
+    // even half: E_k, clean
+    const float2 t0 = axpy_c(g4, p4, w[0]), t1 = axpy_c(-g4, p4, w[0]);
+    const float2 pe = axpy_c(g6 / g2, p6, p2), me = mul_qi<DIR>(axpy_c(-(g6 / g2), p6, p2));
+    const float2 e0 = axpy_c(g2, pe, t0), e2 = axpy_c(-g2, pe, t0), e1 = axpy_c(g2, me, t1), e3 = axpy_c(-g2, me, t1);
+    // odd half: O_k = g1 q_k
+    const float2 a = axpy_c(g5 / g1, p5, p1), b = axpy_c(-(g5 / g1), p5, p1);
+    const float2 c = axpy_c(g7 / g3, p7, p3), d = mul_qi<DIR>(axpy_c(-(g7 / g3), p7, p3));
+    const float2 q0 = axpy_c(g3 / g1, c, a), q2 = mul_qi<DIR>(axpy_c(-(g3 / g1), c, a));
+    const float2 q1 = axpy_c(g3 / g1, d, b), q3 = mul_qi<DIR>(axpy_c(-(g3 / g1), d, b));
+    const float2 s1 = cadd(q1, mul_qi<DIR>(q1)), s3 = cadd(q3, mul_qi<DIR>(q3));
+    w[0] = axpy_c(g1, q0, e0); w[4] = axpy_c(-g1, q0, e0);
+    w[2] = axpy_c(g1, q2, e2); w[6] = axpy_c(-g1, q2, e2);
+    w[1] = axpy_c(g1 * h, s1, e1); w[5] = axpy_c(-(g1 * h), s1, e1);
+    w[3] = axpy_c(g1 * h, s3, e3); w[7] = axpy_c(-(g1 * h), s3, e3);
+}
+
+// ---- FMA form of the cross-thread radix-4 stage with its variable twiddles W128^(q gi), q = 1..3 (forward sign):
+// W128^(q gi) = g_q (1 + i T_q), so w u = g (u + T (i u)).  A zero cosine (q gi = 32) becomes g = 2^-40, T = -2^40, which
+// gives -i u exactly.  Table entry of gi, 12 floats: (-T1, T1, -T2, T2), (-T3, T3, r31, r31), (g2, g2, g1, g1), r31 = g3/g1.
+PTY_DEV void fill_twf(int gi, float* e) {
+    double g[4], T[4];
+    for (int q = 1; q < 4; ++q) {
+        double sn, cs;
+        sincospi(2.0 * (double)(q * gi) / 128.0, &sn, &cs);
+        if ((q * gi) % 64 == 32) cs = 9.094947017729282e-13;
+        g[q] = cs; T[q] = -sn / cs;
+    }
+    e[0] = (float)-T[1]; e[1] = (float)T[1]; e[2] = (float)-T[2]; e[3] = (float)T[2];
+    e[4] = (float)-T[3]; e[5] = (float)T[3]; e[6] = e[7] = (float)(g[3] / g[1]);
+    e[8] = e[9] = (float)g[2]; e[10] = e[11] = (float)g[1];
+}
+// (a0, a1, a2, a3) <- forward radix-4 butterfly of (a0, w1 a1, w2 a2, w3 a3): 11 packed FMAs
+PTY_DEV void bfly4_tw_fma(float4 A, float4 Bq, float4 Cq, float2& a0, float2& a1, float2& a2, float2& a3) {
+    const float2 P1 = make_float2(A.x, A.y), P2 = make_float2(A.z, A.w), P3 = make_float2(Bq.x, Bq.y);
+    const float2 R = make_float2(Bq.z, Bq.w), G2s = make_float2(Cq.x, Cq.y), G1s = make_float2(Cq.z, Cq.w);
+    const float2 p1 = __ffma2_rn(make_float2(a1.y, a1.x), P1, a1);
+    const float2 p2 = __ffma2_rn(make_float2(a2.y, a2.x), P2, a2);
+    const float2 p3 = __ffma2_rn(make_float2(a3.y, a3.x), P3, a3);
+    const float2 t0 = __ffma2_rn(G2s, p2, a0), t1 = __ffma2_rn(make_float2(-G2s.x, -G2s.y), p2, a0);
+    const float2 pp = __ffma2_rn(R, p3, p1);
+    const float2 mm = mul_qi<-1>(__ffma2_rn(make_float2(-R.x, -R.y), p3, p1));
+    a0 = __ffma2_rn(G1s, pp, t0);
+    a2 = __ffma2_rn(make_float2(-G1s.x, -G1s.y), pp, t0);
+    a1 = __ffma2_rn(G1s, mm, t1);
+    a3 = __ffma2_rn(make_float2(-G1s.x, -G1s.y), mm, t1);
+}
+
 // Background work interleaved with a transform: the transforms call bg.tick<K>() at points spread over
 // their arithmetic (K = 0, 1, ... in program order); the kernel bodies use the ticks to fetch the global
 // data of the NEXT pointwise step in small chunks and park it in tensor memory.  The inverse transform
@@ -85,6 +181,27 @@ struct NoBg { template <int K> PTY_DEV void tick() {} };
 template <int DIR, int TB, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg) {
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) bfly4<DIR>(v[n2], v[8 + n2], v[16 + n2], v[24 + n2]);   // -> v[8 k1 + n2]
+#if PTY_FMA_FORM
+    bg.template tick<TB>();
+    {
+        float2 o[32];
+#define PTY_F8(K1)                                                                         \
+        {                                                                                  \
+            float2 w[8];                                                                   \
+            _Pragma("unroll") for (int n2 = 0; n2 < 8; ++n2) w[n2] = v[8 * K1 + n2];       \
+            fft8_pend<K1, DIR>(w);                                                         \
+            _Pragma("unroll") for (int k2 = 0; k2 < 8; ++k2) o[K1 + 4 * k2] = w[k2];       \
+        }
+        PTY_F8(0) bg.template tick<TB + 1>();
+        PTY_F8(1) bg.template tick<TB + 2>();
+        PTY_F8(2) bg.template tick<TB + 3>();
+        PTY_F8(3)
+#undef PTY_F8
+#pragma unroll
+        for (int k = 0; k < 32; ++k) v[k] = o[k];
+        return;
+    }
+#endif
 #define PTY_TW(K1, N2) v[8 * K1 + N2] = mul_w32<K1 * N2, DIR>(v[8 * K1 + N2]);
     PTY_TW(1, 1) PTY_TW(1, 2) PTY_TW(1, 3) PTY_TW(1, 4) PTY_TW(1, 5) PTY_TW(1, 6) PTY_TW(1, 7)
     PTY_TW(2, 1) PTY_TW(2, 2) PTY_TW(2, 3) PTY_TW(2, 4) PTY_TW(2, 5) PTY_TW(2, 6) PTY_TW(2, 7)

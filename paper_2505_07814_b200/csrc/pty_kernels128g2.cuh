@@ -82,13 +82,16 @@ struct G2Smem {
 #ifndef PTY_ABL_SMEM_PAD
 #define PTY_ABL_SMEM_PAD 0      // timing ablation: extra dynamic shared memory (shrinks L1)
 #endif
-    static constexpr size_t bytes = xch_bytes + 128 * sizeof(float2) + 2 * group_bytes + 16 + PTY_ABL_SMEM_PAD;
+    // twf[32][12]: FMA-form constants of the forward radix-4 stage (g2_radix4<-1>)
+    static constexpr size_t twf_bytes = 32 * 12 * sizeof(float);
+    static constexpr size_t bytes = xch_bytes + 128 * sizeof(float2) + 2 * group_bytes + 16 + twf_bytes + PTY_ABL_SMEM_PAD;
 };
 
 struct G2 {
     int tid, t, G, gg, c, smsp;
     float2* X;
     float2* twg;
+    const float4* twf;   // [gi][3] float4: (-T1, T1, -T2, T2), (-T3, T3, r31, r31), (g2, g2, g1, g1)
     float2 *Ey, *Ex, *My, *Mx;
     float* red;
     unsigned tl;     // TMEM address: this thread's lane quarter, first column of the group (256 G)
@@ -122,6 +125,12 @@ PTY_DEV G2 make_g2(unsigned char* smem) {
     c.red = reinterpret_cast<float*>(gt + 512);
     unsigned* tbase = reinterpret_cast<unsigned*>(reinterpret_cast<unsigned char*>(tab + 128) + 2 * G2Smem::group_bytes);
     if ((threadIdx.x >> 5) == 0) tmem_alloc512(tbase);
+    {   // W128^(q gi) = g_q (1 + i T_q), q = 1..3 (forward sign): w u = g (u + T (i u)); a zero cosine (q gi = 32) becomes
+        // g = 2^-40, T = -+2^40, which gives -+i u exactly
+        float* twf = reinterpret_cast<float*>(tbase + 4);
+        c.twf = reinterpret_cast<const float4*>(twf);
+        if (c.tid >= 32 && c.tid < 64) fill_twf(c.tid - 32, twf + 12 * (c.tid - 32));
+    }
     for (int j = c.tid; j < 128; j += 512) {
         float s, co;
         const int gi = j >> 2, qq = j & 3;
@@ -216,6 +225,18 @@ PTY_DEV void g2_item_rows(const KArgs& A, int item, int o, int& row0, int& rx) {
 // DIR < 0: v[8 q + i] -> twiddle W128^(q (8 o + i)) -> radix-4 over q -> v[8 k2 + i]   (forward)
 // DIR > 0: v[8 k2 + i] -> inverse radix-4 over k2 -> conj twiddle -> v[8 q + i]         (inverse)
 template <int DIR> PTY_DEV void g2_radix4(const G2& c, int o, float2 (&v)[32]) {
+#if PTY_FMA_FORM
+    if constexpr (DIR < 0) {
+        // FMA form (pty_fft128.cuh): the three twiddled inputs cost one packed FMA each, their real scales ride on the
+        // butterfly's add/sub pairs: 11 packed FMAs per butterfly instead of 12 scalar + 8 packed instructions
+        const float4* tf = c.twf + 24 * o;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            bfly4_tw_fma(tf[3 * i], tf[3 * i + 1], tf[3 * i + 2], v[i], v[8 + i], v[16 + i], v[24 + i]);
+        }
+        return;
+    }
+#endif
     const float4* tw = reinterpret_cast<const float4*>(c.twg + 32 * o);
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
