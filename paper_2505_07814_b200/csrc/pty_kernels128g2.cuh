@@ -25,6 +25,9 @@
 #ifndef PTY_G2_EARLY
 #define PTY_G2_EARLY 0  // request the first D saved-wave chunks before the park phase's inverse transforms
 #endif
+#ifndef PTY_G2_FLIP
+#define PTY_G2_FLIP 1
+#endif
 #ifndef PTY_G2_D
 #define PTY_G2_D 3      // chunks of saved-wave / object rows in flight in the adjoint's streaming step
 #endif
@@ -388,6 +391,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
     int ry, rx;
     setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
     c.grp_sync();
+    g2_trace(20);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)slot;
     float2 v[32];
@@ -405,6 +409,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
         }
         tmem_wait_st();
     }
+    g2_trace(21);
     bool first = (c.G == 0);
     for (int s = 0; s < A.Nz; ++s) {
         g2_inverse_head(c, v, first);
@@ -412,7 +417,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
         // a3 + a4 (R): psi_{s-1} = fft32^-1, keep it, phi_s = O_b[s] psi_{s-1}, first stage of the forward y transform
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
-            const int o = 2 * c.gg + h;
+            const int o = 2 * c.gg + (TMA || !PTY_G2_FLIP ? h : (h ^ c.G));   // group 1 takes its roles in the opposite order: its object rows are then the ones group 0 read last (L1 hits)
             const float2* obj = A.object + obj_off + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
             const size_t ostride = (size_t)4 * A.W;
             float2 oa[8], ob[8];
@@ -512,6 +517,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
             g2_st_slots(c, o, v);
         }
         tmem_wait_st();
+        g2_trace(23);
     }
     // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2.  I is kept in thread order as pairs, [r / 2][128 o + ky][r & 1]
     // (layout K: register r of role o holds k_x = 8 o + (r & 7) + 32 (r >> 3)): one 8-byte vector RED per two
@@ -531,6 +537,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
             red_add2(Ib + (r >> 1) * NT + 128 * o + c.c, make_float2(p0.x * p0.x + p0.y * p0.y, p1.x * p1.x + p1.y * p1.y));
         }
     }
+    g2_trace(24);
     if (c.G == 0) c.acquireX();      // consume group 1's last release
 }
 
@@ -561,6 +568,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
         tmem_wait_st();
     }
     float acc_ky = 0.f, acc_kx = 0.f, acc_k2 = 0.f;
+    g2_trace(31);
     bool first = (c.G == 0);
     for (int s = A.Nz - 1; s >= 0; --s) {
         g2_inverse_head(c, v, first);
@@ -574,9 +582,15 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
         constexpr int D = PTY_G2_D;
         const float4* psi0 = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 256 * c.gg + c.c;
         float4 pb[D][2];
+        // group 1 streams its two roles in the opposite order: the object rows it reads are then the ones group 0 (same
+        // position, the neighbouring mode) has read last, and they are still in L1
+        const int fl = PTY_G2_FLIP ? c.G : 0;
+        const int pr0 = fl ? 128 : 0, pr1 = 128 - pr0;                      // saved-wave offset of the first / second role
+        const size_t or0 = fl ? (size_t)A.W : 0, or1 = (size_t)A.W - or0;   // object-row offset
+        const unsigned tr0 = fl ? 64u : 0u, tr1 = 64u - tr0;                // TMEM role block
 #define PTY_G2_ISSUE_PSI(J)                                                                               \
         {                                                                                                 \
-            const float4* pp_ = psi0 + 128 * ((J) >> 3) + (size_t)(2 * ((J) & 7)) * NT;                   \
+            const float4* pp_ = psi0 + ((J) >> 3 ? pr1 : pr0) + (size_t)(2 * ((J) & 7)) * NT;             \
             pb[(J) % D][0] = g2_ld_psi(pp_);                                                              \
             pb[(J) % D][1] = g2_ld_psi(pp_ + NT);                                                         \
         }
@@ -594,6 +608,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
             g2_st_own(c, o, v);
         }
         tmem_wait_st();
+        g2_trace(32);
         {
             const size_t ostride = (size_t)4 * A.W;
             const float2* obj0 = A.object + obj_off + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
@@ -603,7 +618,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
             float2 gb[2][4];
 #define PTY_G2_ISSUE_OBJ(J)                                                                               \
             {                                                                                             \
-                const float2* oo_ = obj0 + (size_t)((J) >> 3) * A.W + (size_t)(4 * ((J) & 7)) * ostride;  \
+                const float2* oo_ = obj0 + ((J) >> 3 ? or1 : or0) + (size_t)(4 * ((J) & 7)) * ostride;    \
                 _Pragma("unroll") for (int i = 0; i < 4; ++i) ob[(J) % D][i] = g2_ld_obj(oo_ + (size_t)i * ostride); \
             }
 #if PTY_G2_EARLY
@@ -614,8 +629,8 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
 #define PTY_G2_STEP(J)                                                                                    \
             {                                                                                             \
                 tmem_wait_ld();                                                                           \
-                if ((J) < 15) tmem_ld4(tb0 + 64u * (((J) + 1) >> 3) + 8u * (((J) + 1) & 7), gb[((J) + 1) & 1]); \
-                float2* go_ = gobj0 + (size_t)((J) >> 3) * A.W + (size_t)(4 * ((J) & 7)) * ostride;       \
+                if ((J) < 15) tmem_ld4(tb0 + (((J) + 1) >> 3 ? tr1 : tr0) + 8u * (((J) + 1) & 7), gb[((J) + 1) & 1]); \
+                float2* go_ = gobj0 + ((J) >> 3 ? or1 : or0) + (size_t)(4 * ((J) & 7)) * ostride;         \
                 _Pragma("unroll") for (int i = 0; i < 4; ++i) {                                           \
                     const float4 q_ = pb[(J) % D][i >> 1];                                                \
                     const float2 ps = (i & 1) ? make_float2(q_.z, q_.w) : make_float2(q_.x, q_.y);        \
@@ -623,14 +638,14 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
                     g2_red_obj(go_ + (size_t)i * ostride, cmulc(ps, g_));                                 \
                     gb[(J) & 1][i] = cmulc(ob[(J) % D][i], g_);                                           \
                 }                                                                                         \
-                tmem_st4(tb0 + 64u * ((J) >> 3) + 8u * ((J) & 7), gb[(J) & 1]);                           \
+                tmem_st4(tb0 + ((J) >> 3 ? tr1 : tr0) + 8u * ((J) & 7), gb[(J) & 1]);                     \
                 if ((J) + D < 16) { PTY_G2_ISSUE_PSI((J) + D) PTY_G2_ISSUE_OBJ((J) + D) }                 \
             }
             PTY_G2_ISSUE(0) PTY_G2_ISSUE(1) PTY_G2_ISSUE(2)
             if (D > 3) PTY_G2_ISSUE(3)
             if (D > 4) PTY_G2_ISSUE(4)
             if (D > 5) PTY_G2_ISSUE(5)
-            tmem_ld4(tb0, gb[0]);
+            tmem_ld4(tb0 + tr0, gb[0]);
             PTY_G2_STEP(0) PTY_G2_STEP(1) PTY_G2_STEP(2) PTY_G2_STEP(3) PTY_G2_STEP(4) PTY_G2_STEP(5)
             PTY_G2_STEP(6) PTY_G2_STEP(7) PTY_G2_STEP(8) PTY_G2_STEP(9) PTY_G2_STEP(10) PTY_G2_STEP(11)
             PTY_G2_STEP(12) PTY_G2_STEP(13) PTY_G2_STEP(14) PTY_G2_STEP(15)
@@ -640,6 +655,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
 #undef PTY_G2_ISSUE_PSI
         }
         tmem_wait_st();
+        g2_trace(33);
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
             const int o = 2 * c.gg + h;
@@ -647,6 +663,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
             fft32<-1, 0>(v, bg);
             g2_st_own(c, o, v);
         }
+        g2_trace(34);
         g2_forward_tail(c, v);
         if (s == 0) break;
         // a9, a13 (K): D-sums against the kept spectrum, conj(M), inverse x radix-4, in-place slots
@@ -675,6 +692,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
             g2_st_slots(c, o, v);
         }
         tmem_wait_st();
+        g2_trace(35);
     }
     // a11, a12 (K): g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
     float accy = 0.f, accx = 0.f;
