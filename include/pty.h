@@ -235,7 +235,9 @@ int pty_adam_update(pty_plan* plan, float* theta, const float* grad, float* m, f
 /* End-to-end variant with HOST buffers (pinned memory recommended; plan needs PTY_FLAG_HOST):
  * copies the inputs host->device, runs pty_forward_loss + pty_backward, copies loss and the
  * gradients device->host and synchronises the stream before returning.  Host outputs that are
- * NULL are skipped. */
+ * NULL are skipped.  The measurements (only the loss kernel reads them) travel on a second stream
+ * owned by the plan while the forward kernel runs, ordered behind `stream` by events; with pageable
+ * host memory the copies serialise and the result is the same. */
 int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe,
                   const float* h_positions, const float* h_tilt, const float* h_meas_amp, int32_t B,
                   double* h_loss, void* h_g_object, void* h_g_probe, float* h_g_positions,

@@ -390,6 +390,10 @@ struct pty_plan {
     const void* tm_obj_ptr;
     pty_loss loss_cfg;           // pty_set_loss; mode 0 = plain amplitude sum
     bool sparse_ready;           // the AP forward has put L_sparse into the statistics of this call
+    // pty_grad_host: the measurements travel on a second stream while the forward kernel runs (only the loss reads them)
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_in = nullptr, ev_meas = nullptr;
+    bool wait_meas = false;
     // optional kernel timing (pty_profile)
     bool profiling;
     struct Timed { cudaEvent_t a, b; int which; };
@@ -634,6 +638,10 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
                            d.tilt_mode == 1 ? tilt : (const float*)nullptr, p->at<float2>(p->L.prop), p->at<float2>(p->L.prop) + d.N));
     PTY_CUDA(p, cudaMemsetAsync(A.I, 0, (size_t)B * NN * sizeof(float), st));
     PTY_CUDA(p, launch_fwd(p, A, st));
+    if (p->wait_meas) {      // pty_grad_host: the loss is the first reader of the measurements
+        p->wait_meas = false;
+        PTY_CUDA(p, cudaStreamWaitEvent(st, p->ev_meas, 0));
+    }
     if (paper_loss) {
         const LossCfg cfg = p->loss_dev();
         float* Isum = p->at<float>(p->L.Isum);
@@ -776,6 +784,11 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
             e = cudaFuncSetAttribute(pty_probe_grad128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
     }
     if (e == cudaSuccess) e = cudaMemset(p->ws + L.scalars, 0, 256);
+    if (e == cudaSuccess && (p->d.flags & PTY_FLAG_HOST)) {
+        e = cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_in, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_meas, cudaEventDisableTiming);
+    }
     if (prev_device >= 0 && prev_device != device) cudaSetDevice(prev_device);   // leave the caller's device as it was
     if (e != cudaSuccess) {
         delete p;
@@ -792,7 +805,13 @@ static void drop_timers(pty_plan* p) {
 }
 
 int pty_destroy(pty_plan* plan) {
-    if (plan) drop_timers(plan);
+    if (plan) {
+        drop_timers(plan);
+        DeviceGuard dg(plan->device);
+        if (plan->ev_in) cudaEventDestroy(plan->ev_in);
+        if (plan->ev_meas) cudaEventDestroy(plan->ev_meas);
+        if (plan->copy_stream) cudaStreamDestroy(plan->copy_stream);
+    }
     delete plan;
     return PTY_OK;
 }
@@ -919,7 +938,13 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, con
     PTY_CUDA(plan, cudaMemcpyAsync(dprobe, h_probe, probe_bytes, cudaMemcpyHostToDevice, st));
     if (B) PTY_CUDA(plan, cudaMemcpyAsync(dpos, h_positions, (size_t)B * 8, cudaMemcpyHostToDevice, st));
     if (dtilt) PTY_CUDA(plan, cudaMemcpyAsync(dtilt, h_tilt, tilt_n * 4, cudaMemcpyHostToDevice, st));
-    if (B) PTY_CUDA(plan, cudaMemcpyAsync(dmeas, h_meas_amp, (size_t)B * NN * 4, cudaMemcpyHostToDevice, st));
+    if (B) {   // measurements on the copy stream, behind whatever `st` holds so far; joined before the loss kernel
+        PTY_CUDA(plan, cudaEventRecord(plan->ev_in, st));
+        PTY_CUDA(plan, cudaStreamWaitEvent(plan->copy_stream, plan->ev_in, 0));
+        PTY_CUDA(plan, cudaMemcpyAsync(dmeas, h_meas_amp, (size_t)B * NN * 4, cudaMemcpyHostToDevice, plan->copy_stream));
+        PTY_CUDA(plan, cudaEventRecord(plan->ev_meas, plan->copy_stream));
+        plan->wait_meas = true;
+    }
     rc = run_forward(plan, dobj, dprobe, dpos, dtilt, dmeas, B, plan->d_loss(), nullptr, nullptr, st);
     if (rc != PTY_OK) return rc;
     float2* g_object = plan->at<float2>(plan->L.g_object);
