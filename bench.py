@@ -253,6 +253,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-epoch", action="store_true", help="skip the full-iteration (epoch) timing")
+    ap.add_argument("--plan-flags", type=int, default=0,
+                    help="extra pty_dims.flags for the timed plan (16 = PTY_FLAG_TMA_OBJECT, 32 = PTY_FLAG_PAIR_SUM): "
+                         "opt-in kernel variants, reported in config.plan_flags")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -285,7 +288,7 @@ def main():
     n_used = min(nb_total, args.steps + args.warmup)
     my_batches = [(rank + world * j) % nb_total for j in range(n_used)]
     want_e2e = not args.no_e2e
-    plan = binding.plan_for(cfg, Bmax=B, flags=binding.PTY_FLAG_HOST if want_e2e else 0, device=local)
+    plan = binding.plan_for(cfg, Bmax=B, flags=(binding.PTY_FLAG_HOST if want_e2e else 0) | args.plan_flags, device=local)
     to = lambda x: None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(dev)
     obj_t, probe_t = to(tr["object"]), to(tr["probe"])
     tilt_t = to(tr["tilt"]) if cfg.tilt_mode else None
@@ -438,7 +441,7 @@ def main():
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, B),
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, B, extra={"plan_flags": args.plan_flags} if args.plan_flags else None),
            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "loss": final_loss}
     if e2e:
         out["e2e"] = e2e

@@ -76,6 +76,14 @@ extern "C" {
                                        results.  Needs an even W and a 16-byte aligned `object`, otherwise
                                        the register path runs.  Off by default: measured slower on c4
                                                                                   */
+#define PTY_FLAG_PAIR_SUM     32    /* N = 128, adjoint kernel: sum the g_object contributions of the two
+                                       probe modes a CTA holds (two groups, one position) in a shared-memory
+                                       ring before the one global reduction per pixel -- the on-chip part of
+                                       the crop's adjoint: half the atomics,
+                                       same results up to the summation order.  Needs an even n_obj * M
+                                       (otherwise a CTA's two items can belong to two positions and the
+                                       per-item reductions run).  Off by default: the ring couples the two
+                                       groups' phases and is measured slower      */
 
 /* pty_backward flags */
 #define PTY_BWD_ACCUMULATE     1    /* add into the gradient outputs instead of overwriting    */

@@ -23,7 +23,7 @@ lib = C.CDLL(LIB_PATH)
 
 PTY_OK, PTY_ERR_INVALID_ARG, PTY_ERR_UNSUPPORTED = 0, -1, -2
 PTY_ERR_WORKSPACE, PTY_ERR_CUDA, PTY_ERR_BOUNDS = -3, -4, -5
-PTY_FLAG_SPECTRA, PTY_FLAG_STEP, PTY_FLAG_HOST, PTY_FLAG_AMP_PHASE, PTY_FLAG_TMA_OBJECT = 1, 2, 4, 8, 16
+PTY_FLAG_SPECTRA, PTY_FLAG_STEP, PTY_FLAG_HOST, PTY_FLAG_AMP_PHASE, PTY_FLAG_TMA_OBJECT, PTY_FLAG_PAIR_SUM = 1, 2, 4, 8, 16, 32
 PTY_BWD_ACCUMULATE, PTY_BWD_REUSE_FORWARD = 1, 4
 
 EXPORTS = ["pty_workspace_bytes", "pty_create", "pty_destroy", "pty_forward_loss", "pty_backward",

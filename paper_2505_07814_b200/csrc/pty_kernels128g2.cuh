@@ -25,6 +25,9 @@
 #ifndef PTY_G2_EARLY
 #define PTY_G2_EARLY 0  // request the first D saved-wave chunks before the park phase's inverse transforms
 #endif
+#ifndef PTY_G2_PAIR_NS
+#define PTY_G2_PAIR_NS 4   // chunk slots of the pair-sum ring (8 KB each); measured on c4: 2 -> 6.27 ms, 4 -> 6.13 ms, 8 -> 7.30 ms (L1 shrinks)
+#endif
 #ifndef PTY_G2_FLIP
 #define PTY_G2_FLIP 1
 #endif
@@ -207,6 +210,36 @@ PTY_DEV void g2_ring_fill(G2Ring& r, int rx, int row0) {
         tma_load_3d(r.slots + k * G2Ring::slot_elems, r.tm, rx & ~1, row0 & 3, (row0 >> 2) + G2Ring::ROWS * k, r.full + k);
     }
     r.ppar ^= 1u;
+}
+
+// ------------------------------------------------------------------------------ pair sum of the object gradient (a10)
+// PTY_FLAG_PAIR_SUM: the two groups of a CTA hold two modes of ONE position, so their contributions conj(psi) g to
+// g_object[s, patch] fall on the same pixels.  Group 0 deposits its contribution of every 4-row chunk of the adjoint's
+// streaming step in a shared-memory ring, group 1 adds its own and issues the one reduction: half the atomics.  The
+// ring (NS chunk slots, full / empty mbarriers, one arrival per warp) is a FIFO over the whole kernel; it bounds how far
+// group 0 may run ahead of group 1 (NS chunks), which couples the groups' phases -- the price.
+struct G2Pair {
+    static constexpr int NS = PTY_G2_PAIR_NS;
+    static constexpr int slot_elems = 2 * 4 * 128;                    // [gg][row i][column c] float2
+    static constexpr size_t offset = (G2Smem::bytes + 127) / 128 * 128;
+    static constexpr size_t bytes = offset + (size_t)NS * slot_elems * sizeof(float2) + 2 * NS * sizeof(unsigned long long);
+    float2* slots;
+    unsigned long long *full, *empty;
+    unsigned q;                                                       // chunks passed so far (same count in both groups)
+};
+PTY_DEV G2Pair make_g2_pair(unsigned char* smem) {
+    G2Pair r;
+    r.slots = reinterpret_cast<float2*>(smem + G2Pair::offset);
+    r.full = reinterpret_cast<unsigned long long*>(r.slots + G2Pair::NS * G2Pair::slot_elems);
+    r.empty = r.full + G2Pair::NS;
+    r.q = 0;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < G2Pair::NS; ++k) { mbar_init(r.full + k, 8); mbar_init(r.empty + k, 8); }
+        mbar_init_fence();
+    }
+    __syncthreads();
+    return r;
 }
 
 // crop origin of position b (the same arithmetic as setup_factors: F1 with the clamp of reading R22)
@@ -542,7 +575,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
 }
 
 // ------------------------------------------------------------------------------ adjoint (a7-a13)
-template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int item, int slot, float scl) {
+template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, G2Pair& pr, int item, int slot, float scl) {
     constexpr int N = 128, NT = F128::NT;
     int b, m;
     size_t obj_off;
@@ -584,7 +617,7 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
         float4 pb[D][2];
         // group 1 streams its two roles in the opposite order: the object rows it reads are then the ones group 0 (same
         // position, the neighbouring mode) has read last, and they are still in L1
-        const int fl = PTY_G2_FLIP ? c.G : 0;
+        const int fl = (PTY_G2_FLIP && !PAIR) ? c.G : 0;     // pair sum: both groups must walk the rows in one order
         const int pr0 = fl ? 128 : 0, pr1 = 128 - pr0;                      // saved-wave offset of the first / second role
         const size_t or0 = fl ? (size_t)A.W : 0, or1 = (size_t)A.W - or0;   // object-row offset
         const unsigned tr0 = fl ? 64u : 0u, tr1 = 64u - tr0;                // TMEM role block
@@ -631,12 +664,32 @@ template <bool HAT> PTY_DEV void bwd_body_g2(const KArgs& A, const G2& c, int it
                 tmem_wait_ld();                                                                           \
                 if ((J) < 15) tmem_ld4(tb0 + (((J) + 1) >> 3 ? tr1 : tr0) + 8u * (((J) + 1) & 7), gb[((J) + 1) & 1]); \
                 float2* go_ = gobj0 + ((J) >> 3 ? or1 : or0) + (size_t)(4 * ((J) & 7)) * ostride;         \
+                float2 ct_[4];                                                                            \
                 _Pragma("unroll") for (int i = 0; i < 4; ++i) {                                           \
                     const float4 q_ = pb[(J) % D][i >> 1];                                                \
                     const float2 ps = (i & 1) ? make_float2(q_.z, q_.w) : make_float2(q_.x, q_.y);        \
                     const float2 g_ = gb[(J) & 1][i];                                                     \
-                    g2_red_obj(go_ + (size_t)i * ostride, cmulc(ps, g_));                                 \
+                    ct_[i] = cmulc(ps, g_);                                                               \
                     gb[(J) & 1][i] = cmulc(ob[(J) % D][i], g_);                                           \
+                }                                                                                         \
+                if constexpr (PAIR) {                                                                     \
+                    const unsigned k_ = pr.q % G2Pair::NS, ph_ = (pr.q / G2Pair::NS) & 1u;                \
+                    float2* sl_ = pr.slots + k_ * G2Pair::slot_elems + 512 * c.gg + c.c;                  \
+                    if (c.G == 0) {                                                                       \
+                        mbar_wait(pr.empty + k_, ph_ ^ 1u);                                               \
+                        _Pragma("unroll") for (int i = 0; i < 4; ++i) sl_[128 * i] = ct_[i];              \
+                        __syncwarp();                                                                     \
+                        if (warp_leader()) mbar_arrive(pr.full + k_);                                     \
+                    } else {                                                                              \
+                        mbar_wait(pr.full + k_, ph_);                                                     \
+                        _Pragma("unroll") for (int i = 0; i < 4; ++i)                                     \
+                            g2_red_obj(go_ + (size_t)i * ostride, cadd(ct_[i], sl_[128 * i]));            \
+                        __syncwarp();                                                                     \
+                        if (warp_leader()) mbar_arrive(pr.empty + k_);                                    \
+                    }                                                                                     \
+                    ++pr.q;                                                                               \
+                } else {                                                                                  \
+                    _Pragma("unroll") for (int i = 0; i < 4; ++i) g2_red_obj(go_ + (size_t)i * ostride, ct_[i]); \
                 }                                                                                         \
                 tmem_st4(tb0 + ((J) >> 3 ? tr1 : tr0) + 8u * ((J) & 7), gb[(J) & 1]);                     \
                 if ((J) + D < 16) { PTY_G2_ISSUE_PSI((J) + D) PTY_G2_ISSUE_OBJ((J) + D) }                 \

@@ -116,16 +116,20 @@ __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A
     }
     release_g2(smem);
 }
-template <bool HAT> __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_kernel(const KArgs A) {
-    extern __shared__ __align__(16) unsigned char smem[];
+// PAIR: the two groups of a CTA sum their g_object contributions in shared memory before the one reduction (G2Pair;
+// the host selects it only when every item pair 2x, 2x + 1 holds two modes of one position, i.e. n_obj M is even)
+template <bool HAT, bool PAIR> __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_kernel(const KArgs A) {
+    extern __shared__ __align__(128) unsigned char smem[];
     const G2 c = make_g2(smem);
+    G2Pair pr{};
+    if constexpr (PAIR) pr = make_g2_pair(smem);
     const int n = A.B * A.MT;
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         int item = it + c.G;
 #ifdef PTY_ABL_ONEGROUP
         if (c.G == 1) break;
 #endif
-        bwd_body_g2<HAT>(A, c, min(item, n - 1), item, item < n ? 1.f : 0.f);
+        bwd_body_g2<HAT, PAIR>(A, c, pr, min(item, n - 1), item, item < n ? 1.f : 0.f);
         c.grp_sync();
     }
     release_g2(smem);
@@ -555,8 +559,13 @@ cudaError_t launch_fwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
 cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 1, st);
     if (p->d.N == 128)
-        return A.save_hat ? launch(p, pty_bwd128g2_kernel<true>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A)
-                          : launch(p, pty_bwd128g2_kernel<false>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A);
+    {
+        if ((p->d.flags & PTY_FLAG_PAIR_SUM) && A.MT % 2 == 0)
+            return A.save_hat ? launch(p, pty_bwd128g2_kernel<true, true>, g2_grid(p, A), F128::NT, G2Pair::bytes, 1, st, A)
+                              : launch(p, pty_bwd128g2_kernel<false, true>, g2_grid(p, A), F128::NT, G2Pair::bytes, 1, st, A);
+        return A.save_hat ? launch(p, pty_bwd128g2_kernel<true, false>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A)
+                          : launch(p, pty_bwd128g2_kernel<false, false>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A);
+    }
     return p->d.N == 64 ? launch_bwd_sh<Shape<64>>(p, A, st) : launch_bwd_sh<Shape<256>>(p, A, st);
 }
 // plain 2-D FFT of `items` planes (N = 64, 256): P^ = F[P] / N and g_probe = F^-1[G^_P] / N
@@ -775,9 +784,13 @@ int pty_create(pty_plan** out_plan, const pty_dims* dims, void* workspace, size_
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_fwd128g2_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Ring::bytes);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
+            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Pair::bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Pair::bytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(pty_bwd128g2_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G2Smem::bytes);
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(pty_probe_hat128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F128::smem_bytes);
         if (e == cudaSuccess)

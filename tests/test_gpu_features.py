@@ -343,3 +343,36 @@ def test_tma_flag_falls_back_when_the_object_cannot_be_mapped(pty):
     assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * ref["loss"]
     assert rel_l2(g_obj.cpu().numpy(), ref["g_object"]) <= GRAD_RTOL
     assert plan.status()[0] == 0
+
+
+# ----------------------------------------------------------------------------- on-chip pair sum of the object gradient
+def _pair_sum_case(name):
+    if name == "c3_Nz3_M4":            # one item pair per CTA; 48 chunks per item: the 8-slot ring wraps six times
+        return small_case(3, 6, Nz=3, M=4)
+    if name == "c4_B5":                # the headline shapes: 12 modes = 6 pairs per position
+        return small_case(4, 5)
+    if name == "c3_two_pairs_per_cta":  # 160 pairs on 148 persistent CTAs: the FIFO runs across items
+        return small_case(3, 160, Nz=2, M=2)
+    if name == "c3_tilt_per_position":  # the <HAT = true> adjoint (tilt / dz gradients), full c3 depth
+        idx = synth.minibatch(synth.get_config(3), 1, 512)[:7]     # the positions of test_per_position_tilt_and_dz
+        return make_case(3, "A", idx, tilt_mode=2)
+    if name == "c3_M3_falls_back":     # odd n_obj M: a CTA's two items can sit on two positions -> per-item reductions
+        return small_case(3, 7, Nz=3, M=3)
+    raise KeyError(name)
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("name", ["c3_Nz3_M4", "c4_B5", "c3_two_pairs_per_cta", "c3_tilt_per_position", "c3_M3_falls_back"])
+def test_pair_sum_of_the_object_gradient_matches_the_oracle(pty, name):
+    """PTY_FLAG_PAIR_SUM (the adjoint of the crop): group 0 of every CTA hands its
+    conj(psi) g to group 1 through a shared-memory ring and ONE reduction per pixel and mode pair reaches g_object.
+    Loss and every gradient against the oracle, and g_object against the default per-item reductions."""
+    case = _pair_sum_case(name)
+    cfg = case["cfg"]
+    from test_gpu_parity import check_against_oracle, run_gpu
+    ref = oracle.grad_batch(case["object"], case["probe"], case["positions"], case["tilt"], case["meas"], geom_of(cfg))
+    res = run_gpu(pty, case, flags=pty.PTY_FLAG_PAIR_SUM)
+    check_against_oracle(res, ref, case)
+    plain = run_gpu(pty, case)
+    for k in ("g_object", "g_probe", "g_positions"):
+        assert rel_l2(res[k], plain[k]) <= 1e-5
