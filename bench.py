@@ -253,6 +253,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-epoch", action="store_true", help="skip the full-iteration (epoch) timing")
+    ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
+                    help="replay each step (forward + gradient of one minibatch) as one CUDA graph; auto = on for the "
+                         "launch-bound small configurations 1 and 2 on one GPU")
     ap.add_argument("--plan-flags", type=int, default=0,
                     help="extra pty_dims.flags for the timed plan (16 = PTY_FLAG_TMA_OBJECT, 32 = PTY_FLAG_PAIR_SUM): "
                          "opt-in kernel variants, reported in config.plan_flags")
@@ -326,6 +329,25 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    # Launch-bound small configurations: one CUDA graph per minibatch (the calls are enqueue-only, so a step can be
+    # captured), replayed in the timed region -- one launch call per step instead of eight.
+    use_graph = world == 1 and (args.graph == "on" or (args.graph == "auto" and cfg.c in (1, 2)))
+    step_eager, graph_launches = step, 0
+    if use_graph:
+        step_eager(0)
+        torch.cuda.synchronize()
+        graphs = []
+        for j in range(n_used):
+            g = torch.cuda.CUDAGraph()
+            lc0 = plan.launch_count()
+            with torch.cuda.graph(g):
+                step_eager(j)
+            graph_launches = plan.launch_count() - lc0
+            graphs.append(g)
+
+        def step(i):  # noqa: F811
+            graphs[i % n_used].replay()
+
     for i in range(args.warmup):
         step(i)
     barrier()
@@ -342,12 +364,12 @@ def main():
         e1.record()
         barrier()
         ms_total = e0.elapsed_time(e1)
-        launches = plan.launch_count() - l0
+        launches = graph_launches * args.steps if use_graph else plan.launch_count() - l0
         # per-kernel times for the roofline: the same steps again with the library's per-launch CUDA events on
         # (kept out of the region above: two event records per big launch matter on the launch-bound configs)
         plan.profile(True)
         for i in range(min(args.steps, 20)):
-            step(args.warmup + i)
+            step_eager(args.warmup + i)
         prof = plan.profile_read()
         plan.profile(False)
     if world > 1:
@@ -441,7 +463,8 @@ def main():
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, B, extra={"plan_flags": args.plan_flags} if args.plan_flags else None),
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, B, extra=dict(({"plan_flags": args.plan_flags} if args.plan_flags else {}),
+                                                         **({"cuda_graph": "one graph per step (forward + gradient), replayed"} if use_graph else {}))),
            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "loss": final_loss}
     if e2e:
         out["e2e"] = e2e
