@@ -17,6 +17,13 @@
 #include "pty_port.cuh"
 #endif
 
+#ifndef PTY_DSMEM_PTX
+#define PTY_DSMEM_PTX 1   // N = 256: explicit st.shared::cluster for the tile copy (c5: 23.8 -> 22.9 ms forward)
+#endif
+#ifndef PTY_CLUSTER_RELAXED
+#define PTY_CLUSTER_RELAXED 1   // N = 256: the write-after-read cluster barrier of stage B arrives without a release fence (c5: 22.9 -> 22.2 ms)
+#endif
+
 namespace pty {
 
 // ----------------------------------------------------------------------------- complex helpers
@@ -178,6 +185,20 @@ template <class SH> struct Cta {
 template <class SH> PTY_DEV void sync_all() {
     if (SH::CL > 1) pty_cluster_sync(); else pty_cta_sync();
 }
+// Execution barrier only (write-after-read protection: every thread of the cluster has finished READING the waves into
+// registers; nothing written before it has to become visible), so the arrive carries no release fence.
+template <class SH> PTY_DEV void sync_all_war() {
+#if PTY_CLUSTER_RELAXED
+    if (SH::CL > 1) {
+        asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+        asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+    } else {
+        pty_cta_sync();
+    }
+#else
+    sync_all<SH>();
+#endif
+}
 
 // ----------------------------------------------------------------------------- stage A
 // In::load(cta, n2, line, gline, v) fills v[n1] = element (row = R2 n1 + n2, line) of the input,
@@ -203,6 +224,56 @@ PTY_DEV void stage_a(const Cta<SH>& c, In& in) {
     }
 }
 
+// Transposed exchange of stage B for cluster shapes, CTA of rank RANK: the registers v[it][k2] with k2 / K2D == d go to
+// CTA d, rows [RANK NL, +NL) of its wave.
+template <class SH, int RANK>
+PTY_DEV void stage_b_exchange(const Cta<SH>& c, float2 (&v)[ShapeInfo<SH>::TB][SH::R2]) {
+    using I = ShapeInfo<SH>;
+    static_assert(SH::CL <= 4, "switch in stage_b");
+    constexpr int TP = I::NL + 1, K2D = I::NL / I::R1;          // k2 values per destination
+    static_assert(I::NL % I::R1 == 0 && (I::NL * I::NL) % I::NT == 0, "tile split");
+#pragma unroll
+    for (int rr = 0; rr < SH::CL; ++rr) {
+        const int d = (RANK + rr) % SH::CL;
+        if (rr == 0) {      // own rows: scattered 8-byte stores straight into the wave (odd pitch: conflict-free)
+#pragma unroll
+            for (int it = 0; it < I::TB; ++it) {
+                const int t = it * I::NT + c.tid;
+                const int line = t % I::NL, k1 = t / I::NL;
+#pragma unroll
+                for (int k2 = 0; k2 < I::R2; ++k2)
+                    if (k2 / K2D == d) c.S[(RANK * I::NL + line) * I::PITCH + (k1 + I::R1 * (k2 % K2D))] = v[it][k2];
+            }
+            continue;
+        }
+        float2* tile = c.stg + (rr & 1) * (I::NL * TP);
+#pragma unroll
+        for (int it = 0; it < I::TB; ++it) {
+            const int t = it * I::NT + c.tid;
+            const int line = t % I::NL, k1 = t / I::NL;
+#pragma unroll
+            for (int k2 = 0; k2 < I::R2; ++k2)
+                if (k2 / K2D == d) tile[line * TP + (k1 + I::R1 * (k2 % K2D))] = v[it][k2];
+        }
+        pty_cta_sync();
+        unsigned rbase;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbase)
+                     : "r"((unsigned)__cvta_generic_to_shared(c.S + (size_t)(RANK * I::NL) * I::PITCH)), "r"(d));
+        float2 tv[(I::NL * I::NL) / I::NT];
+#pragma unroll
+        for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
+            const int idx = j * I::NT + c.tid;
+            tv[j] = tile[(idx / I::NL) * TP + idx % I::NL];
+        }
+#pragma unroll
+        for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
+            const int idx = j * I::NT + c.tid;
+            const unsigned a = rbase + (unsigned)(((idx / I::NL) * I::PITCH + idx % I::NL) * sizeof(float2));
+            asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(tv[j].x), "f"(tv[j].y) : "memory");
+        }
+    }
+}
+
 // ----------------------------------------------------------------------------- stage B
 // Reads everything into registers, synchronises, then writes the transposed result:
 // element (old line L_global, k) goes to row L_global, column k of the new orientation,
@@ -219,7 +290,7 @@ PTY_DEV void stage_b(const Cta<SH>& c) {
         for (int n2 = 0; n2 < I::R2; ++n2) v[it][n2] = c.S[(I::R2 * k1 + n2) * I::PITCH + line];
         RegFFT<I::R2, DIR>::run(v[it]);
     }
-    sync_all<SH>();
+    sync_all_war<SH>();
     if constexpr (SH::CL == 1) {
 #pragma unroll
         for (int it = 0; it < I::TB; ++it) {
@@ -234,28 +305,13 @@ PTY_DEV void stage_b(const Cta<SH>& c) {
         // bytes of remote shared memory instead of 32 separate 8-byte words (the scattered form ran at 10 % issue
         // utilisation, stalled on lg_throttle -- profiles/r01_v4_fwd256).  Two tiles alternate, one CTA barrier
         // per destination; destinations start at the own rank so that the four CTAs do not target one peer.
-        constexpr int TP = I::NL + 1, K2D = I::NL / I::R1;          // k2 values per destination
-        static_assert(I::NL % I::R1 == 0 && (I::NL * I::NL) % I::NT == 0, "tile split");
-#pragma unroll
-        for (int rr = 0; rr < SH::CL; ++rr) {
-            const int d = (c.rank + rr) % SH::CL;
-            float2* tile = c.stg + (rr & 1) * (I::NL * TP);
-#pragma unroll
-            for (int it = 0; it < I::TB; ++it) {
-                const int t = it * I::NT + c.tid;
-                const int line = t % I::NL, k1 = t / I::NL;
-#pragma unroll
-                for (int k2 = 0; k2 < I::R2; ++k2)
-                    if (k2 / K2D == d) tile[line * TP + (k1 + I::R1 * (k2 % K2D))] = v[it][k2];
-            }
-            pty_cta_sync();
-            float2* dst = c.Sr[d] + (size_t)(c.rank * I::NL) * I::PITCH;
-#pragma unroll
-            for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
-                const int idx = j * I::NT + c.tid;
-                const int row = idx / I::NL, col = idx % I::NL;
-                dst[row * I::PITCH + col] = tile[row * TP + col];
-            }
+        // The rank is a template parameter of the exchange (a CTA-uniform switch), so the destination of every register
+        // is known at compile time: no predicated-off stores, and the tile for the own CTA is written in place.
+        switch (c.rank) {
+            case 0: stage_b_exchange<SH, 0>(c, v); break;
+            case 1: stage_b_exchange<SH, 1 % SH::CL>(c, v); break;
+            case 2: stage_b_exchange<SH, 2 % SH::CL>(c, v); break;
+            default: stage_b_exchange<SH, 3 % SH::CL>(c, v); break;
         }
     }
     sync_all<SH>();
