@@ -278,7 +278,7 @@ PTY_DEV void stage_b_exchange(const Cta<SH>& c, float2 (&v)[ShapeInfo<SH>::TB][S
 // Reads everything into registers, synchronises, then writes the transposed result:
 // element (old line L_global, k) goes to row L_global, column k of the new orientation,
 // i.e. to CTA k / NL at Sr[.][L_global * PITCH + k % NL].
-template <class SH, int DIR>
+template <class SH, int DIR, bool TR>
 PTY_DEV void stage_b(const Cta<SH>& c) {
     using I = ShapeInfo<SH>;
     float2 v[I::TB][I::R2];
@@ -289,6 +289,20 @@ PTY_DEV void stage_b(const Cta<SH>& c) {
 #pragma unroll
         for (int n2 = 0; n2 < I::R2; ++n2) v[it][n2] = c.S[(I::R2 * k1 + n2) * I::PITCH + line];
         RegFFT<I::R2, DIR>::run(v[it]);
+    }
+    if constexpr (!TR) {
+        // in place: frequency k = k1 + R1 k2 of every line goes to row k of the same line -- local to the CTA, so a
+        // CTA barrier on each side is all it takes (no cluster barrier, no exchange)
+        pty_cta_sync();
+#pragma unroll
+        for (int it = 0; it < I::TB; ++it) {
+            const int t = it * I::NT + c.tid;
+            const int line = t % I::NL, k1 = t / I::NL;
+#pragma unroll
+            for (int k2 = 0; k2 < I::R2; ++k2) c.S[(k1 + I::R1 * k2) * I::PITCH + line] = v[it][k2];
+        }
+        pty_cta_sync();
+        return;
     }
     sync_all_war<SH>();
     if constexpr (SH::CL == 1) {
@@ -317,14 +331,6 @@ PTY_DEV void stage_b(const Cta<SH>& c) {
     sync_all<SH>();
 }
 
-// One full pass: stage A (with its fused input work), stage B, transposed write.
-template <class SH, int DIR, class In>
-PTY_DEV void fft_pass(const Cta<SH>& c, In& in) {
-    stage_a<SH, DIR>(c, in);
-    pty_cta_sync();
-    stage_b<SH, DIR>(c);
-}
-
 // Plain input: the wave itself.
 struct InSmem {
     template <class SH, int R>
@@ -334,5 +340,25 @@ struct InSmem {
         for (int n1 = 0; n1 < R; ++n1) v[n1] = c.S[(I::R2 * n1 + n2) * I::PITCH + line];
     }
 };
+
+// One full pass: stage A (with its fused input work), stage B, and the write-back -- transposed (TR: lines <-> rows,
+// through DSMEM on cluster shapes) or in place.  A 2-D FFT is a transposing pass followed by an in-place pass: real
+// space is held as [y][x line], k space TRANSPOSED as [kx][ky line]; the pointwise k-space steps and every k-space
+// workspace array (P^, Psi, psi^, I, seed weights, G^_P) use that orientation, so ONE exchange per 2-D FFT suffices.
+template <class SH, int DIR, bool TR, class In>
+PTY_DEV void fft_pass(const Cta<SH>& c, In& in) {
+    stage_a<SH, DIR>(c, in);
+    pty_cta_sync();
+    stage_b<SH, DIR, TR>(c);
+}
+// 2-D FFT: real [y][x] -> k space [kx][ky] (DIR < 0) or k space [kx][ky] -> real [y][x] (DIR > 0); `in` supplies the
+// elements in the orientation of the source side.
+template <class SH, int DIR, class In>
+PTY_DEV void fft_2d(const Cta<SH>& c, In& in) {
+    InSmem plain;
+    fft_pass<SH, DIR, true>(c, in);
+    fft_pass<SH, DIR, false>(c, plain);
+}
+
 
 }  // namespace pty

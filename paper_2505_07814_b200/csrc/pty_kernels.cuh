@@ -107,17 +107,19 @@ PTY_DEV void setup_tables(const Cta<SH>& c, const KArgs& A, int b, int& ry, int&
 }
 
 // --------------------------------------------------------------------------- stage-A inputs
+// K-space steps see the wave TRANSPOSED (pty_fft.cuh, fft_2d): row = k_x, line = k_y; every k-space workspace array
+// of this kernel family is stored in that order, [k_x][k_y].
 // a2: E_b . P^ (k space), source = global memory
 struct InProbe {
     const float2* Ph;
     template <class SH, int R>
     PTY_DEV void load(const Cta<SH>& c, int n2, int, int gline, float2 (&v)[R]) {
         using I = ShapeInfo<SH>;
-        const float2 exl = c.Ex[gline];
+        const float2 eyl = c.Ey[gline];
 #pragma unroll
         for (int n1 = 0; n1 < R; ++n1) {
             const int row = I::R2 * n1 + n2;
-            v[n1] = cmul(cmul(ldg2(Ph + row * I::N + gline), c.Ey[row]), exl);
+            v[n1] = cmul(cmul(ldg2(Ph + row * I::N + gline), c.Ex[row]), eyl);
         }
     }
 };
@@ -143,17 +145,17 @@ struct InFwdObj {
     }
 };
 
-// a4: multiply the spectrum by the propagator M = My[row] Mx[line] (/N^2); optionally keep it
+// a4: multiply the spectrum by the propagator M = Mx[row] My[line] (/N^2); optionally keep it
 struct InFwdProp {
     float2* save;   // ws_hat[b][m][s] or null
     template <class SH, int R>
     PTY_DEV void load(const Cta<SH>& c, int n2, int line, int gline, float2 (&v)[R]) {
         using I = ShapeInfo<SH>;
-        const float2 mxl = c.Mx[gline];
+        const float2 myl = c.My[gline];
 #pragma unroll
         for (int n1 = 0; n1 < R; ++n1) {
             const int row = I::R2 * n1 + n2;
-            const float2 w = cmul(c.S[row * I::PITCH + line], cmul(c.My[row], mxl));
+            const float2 w = cmul(c.S[row * I::PITCH + line], cmul(c.Mx[row], myl));
             if (save) st_stream2(save + row * I::N + gline, w);
             v[n1] = w;
         }
@@ -217,8 +219,8 @@ struct InBwdProp {
     template <class SH, int R>
     PTY_DEV void load(const Cta<SH>& c, int n2, int line, int gline, float2 (&v)[R]) {
         using I = ShapeInfo<SH>;
-        const float2 mxl = c.Mx[gline];
-        const float kxl = kp_of<I::N>(gline);
+        const float2 myl = c.My[gline];
+        const float kyl = kp_of<I::N>(gline);
 #pragma unroll
         for (int n1 = 0; n1 < R; ++n1) {
             const int row = I::R2 * n1 + n2;
@@ -226,12 +228,12 @@ struct InBwdProp {
             if (hat) {
                 const float2 hs = ld_stream2(hat + row * I::N + gline);
                 const float d = hs.x * g.y - hs.y * g.x;       // Im(conj(psi^) g^)
-                const float kyr = kp_of<I::N>(row);
-                acc_ky += d * kyr;
-                acc_kx += d * kxl;
-                acc_k2 += d * (kyr * kyr + kxl * kxl);
+                const float kxr = kp_of<I::N>(row);
+                acc_ky += d * kyl;
+                acc_kx += d * kxr;
+                acc_k2 += d * (kyl * kyl + kxr * kxr);
             }
-            v[n1] = cmulc(cmul(c.My[row], mxl), g);
+            v[n1] = cmulc(cmul(c.Mx[row], myl), g);
         }
     }
 };
@@ -266,22 +268,18 @@ PTY_DEV void fwd_body(const KArgs& A, const Cta<SH>& c, int item) {
     setup_tables(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)item;
-    InSmem plain;
     {   // psi_0 = F^-1[E . P^]
         InProbe in{A.probe_hat + (size_t)m * NN};
-        fft_pass<SH, +1>(c, in);
-        fft_pass<SH, +1>(c, plain);
+        fft_2d<SH, +1>(c, in);
     }
     for (int s = 0; s < A.Nz; ++s) {
         InFwdObj in{A.object + obj_off + ((size_t)s * A.H + ry) * A.W + rx, A.W, A.ws_psi + (bm * A.Nz + s) * NN};
-        fft_pass<SH, -1>(c, in);
-        fft_pass<SH, -1>(c, plain);
+        fft_2d<SH, -1>(c, in);
         if (s == A.Nz - 1) break;
         InFwdProp ip{A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + s) * NN : nullptr};
-        fft_pass<SH, +1>(c, ip);
-        fft_pass<SH, +1>(c, plain);
+        fft_2d<SH, +1>(c, ip);
     }
-    // a5: Psi = F[phi_Nz] (unitary), I += |Psi|^2
+    // a5: Psi = F[phi_Nz] (unitary), I += |Psi|^2; both in the transposed k-space order [k_x][k_y]
     float2* Psi = A.ws_Psi + bm * NN;
     float* Ib = A.I + (size_t)b * NN;
 #pragma unroll 4
@@ -306,22 +304,18 @@ PTY_DEV void bwd_body(const KArgs& A, const Cta<SH>& c, int item) {
     setup_tables(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)item;
-    InSmem plain;
     {   // B1, B2
         InSeed in{A.ws_Psi + bm * NN, A.seed_w + (size_t)b * NN};
-        fft_pass<SH, +1>(c, in);
-        fft_pass<SH, +1>(c, plain);
+        fft_2d<SH, +1>(c, in);
     }
     InBwdProp ip{nullptr, 0.f, 0.f, 0.f};
     for (int s = A.Nz - 1; s >= 0; --s) {
         const size_t off = obj_off + ((size_t)s * A.H + ry) * A.W + rx;
         InBwdObj in{A.object + off, A.W, A.ws_psi + (bm * A.Nz + s) * NN, A.g_object + off};
-        fft_pass<SH, -1>(c, in);
-        fft_pass<SH, -1>(c, plain);
+        fft_2d<SH, -1>(c, in);
         if (s == 0) break;
         ip.hat = A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + (s - 1)) * NN : nullptr;
-        fft_pass<SH, +1>(c, ip);
-        fft_pass<SH, +1>(c, plain);
+        fft_2d<SH, +1>(c, ip);
     }
     // B6, B7: g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
     const float2* Ph = A.probe_hat + (size_t)m * NN;
@@ -332,12 +326,12 @@ PTY_DEV void bwd_body(const KArgs& A, const Cta<SH>& c, int item) {
         const int idx = it * I::NT + c.tid;
         const int row = idx / I::NL, line = idx % I::NL, gline = c.rank * I::NL + line;
         const float2 g = c.S[row * I::PITCH + line];
-        const float2 e = cmul(c.Ey[row], c.Ex[gline]);           // E / N
+        const float2 e = cmul(c.Ex[row], c.Ey[gline]);           // E / N (row = k_x, line = k_y)
         red_add2(GP + row * N + gline, cmulc(e, g));
         const float2 ep = cmul(e, ldg2(Ph + row * N + gline));
         const float t = g.x * ep.y - g.y * ep.x;                 // Im(conj(g^_0) E P^)
-        accy += kp_of<N>(row) * t;
-        accx += kp_of<N>(gline) * t;
+        accy += kp_of<N>(gline) * t;
+        accx += kp_of<N>(row) * t;
     }
     block_accumulate(c, 0, accy);
     block_accumulate(c, 1, accx);
@@ -375,9 +369,7 @@ PTY_DEV void fft2_body(const float2* src, float2* dst, float scale, int accumula
     pty_cta_sync();
     const size_t NN = (size_t)N * N;
     InGlobal in{src + (size_t)item * NN};
-    InSmem plain;
-    fft_pass<SH, DIR>(c, in);
-    fft_pass<SH, DIR>(c, plain);
+    fft_2d<SH, DIR>(c, in);          // DIR < 0: natural [y][x] -> transposed [k_x][k_y]; DIR > 0: the reverse
     float2* out = dst + (size_t)item * NN;
     for (int it = 0; it < I::SWEEP; ++it) {
         const int idx = it * I::NT + c.tid;

@@ -660,17 +660,15 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
             PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss));
             PTY_CUDA(p, launch(p, pty_seed_kernel<true>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, (int)B, cfg, (const double*)p->d_stats(), (const float*)Isum, (const float*)Imsum, A.seed_w));
         } else {
-            PTY_CUDA(p, launch(p, pty_loss_sums_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, cfg, p->d_stats(), loss_per_pos, Isum, Imsum, (float*)nullptr));
+            PTY_CUDA(p, launch(p, pty_loss_sums_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, cfg, p->d_stats(), loss_per_pos, Isum, Imsum, intensity));
             PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss));
             PTY_CUDA(p, launch(p, pty_seed_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, (int)B, cfg, (const double*)p->d_stats(), (const float*)Isum, (const float*)Imsum, A.seed_w));
         }
     } else if (d.N == 128) {
         PTY_CUDA(p, launch(p, pty_loss_seed128_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, loss, loss_per_pos, A.seed_w, intensity));
     } else {
-        PTY_CUDA(p, launch(p, pty_loss_seed_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, loss, loss_per_pos, A.seed_w));
+        PTY_CUDA(p, launch(p, pty_loss_seed_kernel, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, loss, loss_per_pos, A.seed_w, intensity));
     }
-    if (intensity && d.N != 128)
-        PTY_CUDA(p, cudaMemcpyAsync(intensity, A.I, (size_t)B * NN * sizeof(float), cudaMemcpyDeviceToDevice, st));
     p->fwd_valid = true;
     p->f_object = object; p->f_probe = probe; p->f_positions = positions; p->f_tilt = tilt; p->f_meas = meas;
     p->f_B = B;

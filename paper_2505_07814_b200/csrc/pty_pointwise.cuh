@@ -34,7 +34,7 @@ PTY_DEV double block_sum_256(double v, double* part) {      // 256 threads; resu
 // Visits every detector pixel of one position once: f(I, a, w_index, natural_index).
 // TORD (N = 128): I is in the forward kernel's thread order, pairs [r / 2][128 o + ky][r & 1]; the measured amplitudes
 // (natural order) pass through a 32-row shared tile; w_index is the adjoint kernel's thread order [r][128 o + ky].
-// Otherwise I, a and the seed weights are all in natural order.  256 threads.
+// Otherwise I and the seed weights are transposed, [k_x][k_y], and a is natural.  256 threads.
 template <bool TORD, class F>
 PTY_DEV void sweep_position(const float* __restrict__ Ib, const float* __restrict__ ab, int N, float (*tile)[129], F&& f) {
     const int t = threadIdx.x;
@@ -58,24 +58,33 @@ PTY_DEV void sweep_position(const float* __restrict__ Ib, const float* __restric
             __syncthreads();
         }
     } else {
-        for (int i = t; i < N * N; i += 256) f(__ldg(Ib + i), __ldg(ab + i), i, i);
+        // N = 64 / 256: I and the seed weights are in the transposed k-space order [k_x][k_y] of the shared-memory-pass
+        // kernels (pty_fft.cuh, fft_2d); the measured amplitudes are natural, [k_y][k_x]
+        for (int i = t; i < N * N; i += 256) {
+            const int ky = i / N, kx = i - ky * N, ti = kx * N + ky;
+            f(__ldg(Ib + ti), __ldg(ab + i), ti, i);
+        }
     }
 }
 
 // a6 + a7, plain amplitude sum (north_star; reading R13), N = 64 / 256: L_b = sum_k (sqrt(I) - a)^2 and the seed
-// weights w = 2 (1 - a / sqrt(I)) / N (0 where I = 0, R14) in natural order.  One block per position.
+// weights w = 2 (1 - a / sqrt(I)) / N (0 where I = 0, R14) in the order of I; optionally I in natural order.  One block
+// per position.
 __global__ void __launch_bounds__(256) pty_loss_seed_kernel(const float* __restrict__ I, const float* __restrict__ a, int N,
-                                                           double* loss, float* loss_per_pos, float* __restrict__ seed_w) {
+                                                           double* loss, float* loss_per_pos, float* __restrict__ seed_w,
+                                                           float* __restrict__ intensity) {
     __shared__ double part[8];
     const int b = blockIdx.x;
     const size_t NN = (size_t)N * N;
     float* Wb = seed_w + (size_t)b * NN;
     const float invN = 1.0f / (float)N;
     float acc = 0.f;
-    sweep_position<false>(I + (size_t)b * NN, a + (size_t)b * NN, N, nullptr, [&](float iv, float av, int wi, int) {
+    float* out = intensity ? intensity + (size_t)b * NN : nullptr;
+    sweep_position<false>(I + (size_t)b * NN, a + (size_t)b * NN, N, nullptr, [&](float iv, float av, int wi, int nat) {
         const float d = sqrtf(iv) - av;
         acc += d * d;
         Wb[wi] = iv > 1e-30f ? 2.0f * (1.0f - av * rsqrtf(iv)) * invN : 0.f;
+        if (out) out[nat] = iv;
     });
     const double s = block_sum_256((double)acc, part);
     if (threadIdx.x == 0) {
@@ -102,7 +111,7 @@ __global__ void __launch_bounds__(256) pty_loss_sums_kernel(const float* __restr
         s += d * d; sa += av; sa2 += a2;
         sp += a2 * logf(iv + cfg.eps) - iv;
         if (pacbed) { red_add(Isum + nat, iv); red_add(Imsum + nat, a2); }
-        if (TORD && out) out[nat] = iv;
+        if (out) out[nat] = iv;
     });
     const double S = block_sum_256((double)s, part), A = block_sum_256((double)sa, part),
                  A2 = block_sum_256((double)sa2, part), P = block_sum_256((double)sp, part);
