@@ -20,6 +20,9 @@
 #ifndef PTY_DSMEM_PTX
 #define PTY_DSMEM_PTX 1   // N = 256: explicit st.shared::cluster for the tile copy (c5: 23.8 -> 22.9 ms forward)
 #endif
+#ifndef PTY_STAGE_A_UNROLL
+#define PTY_STAGE_A_UNROLL 1   // both tasks of a thread in flight in stage A (c5: +2 %)
+#endif
 #ifndef PTY_CLUSTER_RELAXED
 #define PTY_CLUSTER_RELAXED 1   // N = 256: the write-after-read cluster barrier of stage B arrives without a release fence (c5: 22.9 -> 22.2 ms)
 #endif
@@ -206,7 +209,11 @@ template <class SH> PTY_DEV void sync_all_war() {
 template <class SH, int DIR, class In>
 PTY_DEV void stage_a(const Cta<SH>& c, In& in) {
     using I = ShapeInfo<SH>;
+#if PTY_STAGE_A_UNROLL
+#pragma unroll
+#else
 #pragma unroll 1
+#endif
     for (int it = 0; it < I::TA; ++it) {
         const int t = it * I::NT + c.tid;
         const int line = t % I::NL, n2 = t / I::NL;
