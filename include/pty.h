@@ -251,6 +251,16 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe,
                   double* h_loss, void* h_g_object, void* h_g_probe, float* h_g_positions,
                   float* h_g_tilt, void* stream);
 
+/* The same call without the final synchronisation: everything is enqueued on `stream` (and the plan's copy
+ * stream) and the host outputs are valid after pty_grad_host_wait(plan).  Two plans on two streams fed alternately
+ * overlap one minibatch's copies with the other's kernels (bench.py's end-to-end number).  The host buffers must
+ * stay untouched, and pinned for any overlap to happen, until the wait returns. */
+int pty_grad_host_async(pty_plan* plan, const void* h_object, const void* h_probe,
+                  const float* h_positions, const float* h_tilt, const float* h_meas_amp, int32_t B,
+                  double* h_loss, void* h_g_object, void* h_g_probe, float* h_g_positions,
+                  float* h_g_tilt, void* stream);
+int pty_grad_host_wait(pty_plan* plan);
+
 /* Synchronises the plan's last stream and returns PTY_OK, PTY_ERR_BOUNDS or PTY_ERR_CUDA.
  * device_flags (host, may be NULL) receives the raw sticky flag word and clears it. */
 int pty_status(pty_plan* plan, int32_t* device_flags);

@@ -29,8 +29,9 @@ PTY_BWD_ACCUMULATE, PTY_BWD_REUSE_FORWARD = 1, 4
 EXPORTS = ["pty_workspace_bytes", "pty_create", "pty_destroy", "pty_forward_loss", "pty_backward",
            "pty_step", "pty_adam_update", "pty_grad_host", "pty_status", "pty_profile",
            "pty_profile_read", "pty_set_loss", "pty_loss_terms", "pty_forward_loss_ap", "pty_backward_ap",
-           "pty_step_ap", "pty_constrain", "pty_rz_filter_object", "pty_launch_count", "pty_last_error", "pty_version"]
-_INT_RETURNS = EXPORTS[:18]
+           "pty_step_ap", "pty_constrain", "pty_rz_filter_object", "pty_grad_host_async", "pty_grad_host_wait",
+           "pty_launch_count", "pty_last_error", "pty_version"]
+_INT_RETURNS = EXPORTS[:20]
 
 
 class pty_dims(C.Structure):
@@ -81,6 +82,8 @@ lib.pty_step.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.POINTER(pty_
 lib.pty_adam_update.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_size_t, C.c_float, C.c_float, C.c_float,
                                 C.c_float, C.c_int32, _vp]
 lib.pty_grad_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, _vp, _vp, _vp, _vp, _vp, _vp]
+lib.pty_grad_host_async.argtypes = lib.pty_grad_host.argtypes
+lib.pty_grad_host_wait.argtypes = [_vp]
 lib.pty_status.argtypes = [_vp, C.POINTER(C.c_int32)]
 lib.pty_profile.argtypes = [_vp, C.c_int32]
 lib.pty_profile_read.argtypes = [_vp, C.POINTER(C.c_float), C.POINTER(C.c_int32), C.POINTER(C.c_float),
@@ -247,13 +250,17 @@ class Plan:
                                         _ptr(v, torch.float32, "cuda"), n, lr, beta1, beta2, eps, t, _stream()))
 
     def grad_host(self, h_obj, h_probe, h_positions, h_tilt, h_meas_amp, h_loss, h_g_object, h_g_probe=None,
-                  h_g_positions=None, h_g_tilt=None):
-        self._check(lib.pty_grad_host(
+                  h_g_positions=None, h_g_tilt=None, wait=True):
+        """wait=False: pty_grad_host_async (enqueue only); call grad_host_wait() before reading the outputs."""
+        self._check((lib.pty_grad_host if wait else lib.pty_grad_host_async)(
             self._h, _ptr(h_obj, torch.complex64, "cpu"), _ptr(h_probe, torch.complex64, "cpu"),
             _ptr(h_positions, torch.float32, "cpu"), _ptr(h_tilt, torch.float32, "cpu"),
             _ptr(h_meas_amp, torch.float32, "cpu"), h_positions.shape[0], _ptr(h_loss, torch.float64, "cpu"),
             _ptr(h_g_object, torch.complex64, "cpu"), _ptr(h_g_probe, torch.complex64, "cpu"),
             _ptr(h_g_positions, torch.float32, "cpu"), _ptr(h_g_tilt, torch.float32, "cpu"), _stream()))
+
+    def grad_host_wait(self):
+        self._check(lib.pty_grad_host_wait(self._h))
 
     def status(self):
         flags = C.c_int32(0)

@@ -929,9 +929,9 @@ int pty_step(pty_plan* plan, void* object, void* probe, float* positions, float*
     return PTY_OK;
 }
 
-int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, const float* h_positions,
-                  const float* h_tilt, const float* h_meas_amp, int32_t B, double* h_loss, void* h_g_object,
-                  void* h_g_probe, float* h_g_positions, float* h_g_tilt, void* stream) {
+static int grad_host_impl(pty_plan* plan, const void* h_object, const void* h_probe, const float* h_positions,
+                          const float* h_tilt, const float* h_meas_amp, int32_t B, double* h_loss, void* h_g_object,
+                          void* h_g_probe, float* h_g_positions, float* h_g_tilt, void* stream, bool wait) {
     int rc = check_batch(plan, h_object, h_probe, h_positions, h_tilt, h_meas_amp, B);
     if (rc != PTY_OK) return rc;
     DeviceGuard dg(plan->device);
@@ -970,7 +970,28 @@ int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, con
     if (h_g_probe) PTY_CUDA(plan, cudaMemcpyAsync(h_g_probe, g_probe, probe_bytes, cudaMemcpyDeviceToHost, st));
     if (h_g_positions && B) PTY_CUDA(plan, cudaMemcpyAsync(h_g_positions, g_pos, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
     if (h_g_tilt && dtilt) PTY_CUDA(plan, cudaMemcpyAsync(h_g_tilt, g_tilt, tilt_n * 4, cudaMemcpyDeviceToHost, st));
-    PTY_CUDA(plan, cudaStreamSynchronize(st));
+    if (wait) PTY_CUDA(plan, cudaStreamSynchronize(st));
+    return PTY_OK;
+}
+
+int pty_grad_host(pty_plan* plan, const void* h_object, const void* h_probe, const float* h_positions,
+                  const float* h_tilt, const float* h_meas_amp, int32_t B, double* h_loss, void* h_g_object,
+                  void* h_g_probe, float* h_g_positions, float* h_g_tilt, void* stream) {
+    return grad_host_impl(plan, h_object, h_probe, h_positions, h_tilt, h_meas_amp, B, h_loss, h_g_object, h_g_probe,
+                          h_g_positions, h_g_tilt, stream, true);
+}
+
+int pty_grad_host_async(pty_plan* plan, const void* h_object, const void* h_probe, const float* h_positions,
+                        const float* h_tilt, const float* h_meas_amp, int32_t B, double* h_loss, void* h_g_object,
+                        void* h_g_probe, float* h_g_positions, float* h_g_tilt, void* stream) {
+    return grad_host_impl(plan, h_object, h_probe, h_positions, h_tilt, h_meas_amp, B, h_loss, h_g_object, h_g_probe,
+                          h_g_positions, h_g_tilt, stream, false);
+}
+
+int pty_grad_host_wait(pty_plan* plan) {
+    if (!plan) return PTY_ERR_INVALID_ARG;
+    DeviceGuard dg(plan->device);
+    PTY_CUDA(plan, cudaStreamSynchronize(plan->last_stream));
     return PTY_OK;
 }
 

@@ -363,6 +363,42 @@ def test_grad_host_end_to_end(pty):
     assert rel_l2(h_gq.numpy(), ref["g_positions"]) <= GRAD_RTOL
 
 
+def test_grad_host_async_two_plans_on_two_streams(pty):
+    """pty_grad_host_async / pty_grad_host_wait: two plans fed alternately on two streams (bench.py's end-to-end
+    pipeline); each minibatch's host results against the oracle."""
+    cfg = synth.get_config(1)
+    cases = [make_case(1, "A", synth.minibatch(cfg, j, cfg.B)) for j in (0, 1, 2)]
+    refs = [oracle_grad(c) for c in cases]
+    pin = lambda x: torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
+    plans = [pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, cfg.B, cfg.dz, cfg.lam, cfg.dx, flags=pty.PTY_FLAG_HOST)
+             for _ in range(2)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    h_in = [(pin(c["object"]), pin(c["probe"]), pin(c["positions"]), pin(c["meas"])) for c in cases]
+    outs = [(torch.zeros(1, dtype=torch.float64).pin_memory(),
+             torch.zeros(cases[0]["object"].shape, dtype=torch.complex64).pin_memory(),
+             torch.zeros(cases[0]["probe"].shape, dtype=torch.complex64).pin_memory(),
+             torch.zeros(cfg.B, 2).pin_memory()) for _ in range(2)]
+
+    def check(i):
+        k = i & 1
+        plans[k].grad_host_wait()
+        h_loss, h_go, h_gp, h_gq = outs[k]
+        ref = refs[i % 3]
+        assert abs(h_loss[0].item() - ref["loss"]) <= LOSS_RTOL * ref["loss"]
+        assert rel_l2(h_go.numpy(), ref["g_object"]) <= GRAD_RTOL
+        assert rel_l2(h_gp.numpy(), ref["g_probe"]) <= GRAD_RTOL
+        assert rel_l2(h_gq.numpy(), ref["g_positions"]) <= GRAD_RTOL
+
+    for i in range(6):
+        k = i & 1
+        o, p, q, m = h_in[i % 3]
+        with torch.cuda.stream(streams[k]):
+            plans[k].grad_host(o, p, q, None, m, *outs[k], wait=False)
+        if i > 0:
+            check(i - 1)
+    check(5)
+
+
 def test_backward_never_reuses_a_stale_forward(pty):
     """forward, then an in-place change of the object (same pointer), then backward.  Without
     PTY_BWD_REUSE_FORWARD the gradient must be the fresh one; pty_adam_update cancels the saved state even if
