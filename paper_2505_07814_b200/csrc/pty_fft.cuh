@@ -358,14 +358,73 @@ PTY_DEV void fft_pass(const Cta<SH>& c, In& in) {
     pty_cta_sync();
     stage_b<SH, DIR, TR>(c);
 }
-// 2-D FFT: real [y][x] -> k space [kx][ky] (DIR < 0) or k space [kx][ky] -> real [y][x] (DIR > 0); `in` supplies the
-// elements in the orientation of the source side.
-template <class SH, int DIR, class In>
-PTY_DEV void fft_2d(const Cta<SH>& c, In& in) {
-    InSmem plain;
-    fft_pass<SH, DIR, true>(c, in);
-    fft_pass<SH, DIR, false>(c, plain);
+// Stage B of an in-place pass, the pointwise step that follows the 2-D FFT, and stage A of the NEXT 2-D FFT's
+// transposing pass, fused in registers.  All passes run over the slow index, and with R1 == R2 the frequencies a
+// stage-B task (line, k1) produces, rows k1 + R1 k2, are exactly the rows R2 n1 + n2 (n1 = k2, n2 = k1) that one
+// stage-A task of the next transform consumes: the values never go back to shared memory in between (one store, one
+// load and one CTA barrier less per 2-D FFT).  op.apply(c, n2, line, gline, v) transforms v[n1] = element
+// (row R2 n1 + n2, line) in place.  Reads (row blocks) and writes (row combs) of different tasks overlap, hence the
+// barrier between them.
+template <class SH, int DIRB, int DIRA, class Op>
+PTY_DEV void stage_b_op_a(const Cta<SH>& c, Op& op) {
+    using I = ShapeInfo<SH>;
+    static_assert(I::R1 == I::R2, "fused stage B -> stage A needs a square radix split");
+    float2 v[I::TB][I::R2];
+#pragma unroll
+    for (int it = 0; it < I::TB; ++it) {
+        const int t = it * I::NT + c.tid;
+        const int line = t % I::NL, k1 = t / I::NL;
+#pragma unroll
+        for (int n2 = 0; n2 < I::R2; ++n2) v[it][n2] = c.S[(I::R2 * k1 + n2) * I::PITCH + line];
+        RegFFT<I::R2, DIRB>::run(v[it]);
+        op.apply(c, k1, line, c.rank * I::NL + line, v[it]);
+        RegFFT<I::R1, DIRA>::run(v[it]);
+#pragma unroll
+        for (int kk = 1; kk < I::R1; ++kk) {
+            float2 w = c.tw[k1 * kk];
+            if (DIRA > 0) w.y = -w.y;
+            v[it][kk] = cmul(v[it][kk], w);
+        }
+    }
+    pty_cta_sync();
+#pragma unroll
+    for (int it = 0; it < I::TB; ++it) {
+        const int t = it * I::NT + c.tid;
+        const int line = t % I::NL, k1 = t / I::NL;
+#pragma unroll
+        for (int kk = 0; kk < I::R1; ++kk) c.S[(I::R2 * kk + k1) * I::PITCH + line] = v[it][kk];
+    }
 }
 
+// A chain of 2-D FFTs with pointwise steps between them:
+//   fft_begin<DIR>(in)        first transform: transposing pass (inputs from `in`), stage A of the in-place pass
+//   fft_link<DIRB, DIRA>(op)  finishes transform DIRB, applies `op`, runs transform DIRA up to the same point
+//   fft_end<DIR>()            finishes the last transform (plain in-place stage B)
+// Orientation: real [y][x] -> k space [kx][ky] (DIR < 0) and back (DIR > 0); `in` / `op` see the source side.
+template <class SH, int DIR, class In>
+PTY_DEV void fft_begin(const Cta<SH>& c, In& in) {
+    InSmem plain;
+    fft_pass<SH, DIR, true>(c, in);
+    stage_a<SH, DIR>(c, plain);
+    pty_cta_sync();
+}
+template <class SH, int DIRB, int DIRA, class Op>
+PTY_DEV void fft_link(const Cta<SH>& c, Op& op) {
+    InSmem plain;
+    stage_b_op_a<SH, DIRB, DIRA>(c, op);
+    pty_cta_sync();
+    stage_b<SH, DIRA, true>(c);
+    stage_a<SH, DIRA>(c, plain);
+    pty_cta_sync();
+}
+template <class SH, int DIR>
+PTY_DEV void fft_end(const Cta<SH>& c) {
+    stage_b<SH, DIR, false>(c);
+}
+template <class SH, int DIR, class In>
+PTY_DEV void fft_2d(const Cta<SH>& c, In& in) {
+    fft_begin<SH, DIR>(c, in);
+    fft_end<SH, DIR>(c);
+}
 
 }  // namespace pty

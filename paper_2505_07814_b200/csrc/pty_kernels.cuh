@@ -129,8 +129,9 @@ struct InFwdObj {
     const float2* obj;   // object + s*H*W + ry*W + rx
     int W;
     float2* save;        // ws_psi[b][m][s]
+    // v[n1] = psi_{s-1}(row R2 n1 + n2, line) on entry (fused step, pty_fft.cuh stage_b_op_a), phi_s on return
     template <class SH, int R>
-    PTY_DEV void load(const Cta<SH>& c, int n2, int line, int gline, float2 (&v)[R]) {
+    PTY_DEV void apply(const Cta<SH>&, int n2, int, int gline, float2 (&v)[R]) {
         using I = ShapeInfo<SH>;
         float2 o[R];
 #pragma unroll
@@ -138,9 +139,8 @@ struct InFwdObj {
 #pragma unroll
         for (int n1 = 0; n1 < R; ++n1) {
             const int row = I::R2 * n1 + n2;
-            const float2 w = c.S[row * I::PITCH + line];
-            st_stream2(save + row * I::N + gline, w);
-            v[n1] = cmul(w, o[n1]);
+            st_stream2(save + row * I::N + gline, v[n1]);
+            v[n1] = cmul(v[n1], o[n1]);
         }
     }
 };
@@ -149,13 +149,13 @@ struct InFwdObj {
 struct InFwdProp {
     float2* save;   // ws_hat[b][m][s] or null
     template <class SH, int R>
-    PTY_DEV void load(const Cta<SH>& c, int n2, int line, int gline, float2 (&v)[R]) {
+    PTY_DEV void apply(const Cta<SH>& c, int n2, int, int gline, float2 (&v)[R]) {
         using I = ShapeInfo<SH>;
         const float2 myl = c.My[gline];
 #pragma unroll
         for (int n1 = 0; n1 < R; ++n1) {
             const int row = I::R2 * n1 + n2;
-            const float2 w = cmul(c.S[row * I::PITCH + line], cmul(c.Mx[row], myl));
+            const float2 w = cmul(v[n1], cmul(c.Mx[row], myl));
             if (save) st_stream2(save + row * I::N + gline, w);
             v[n1] = w;
         }
@@ -189,7 +189,7 @@ struct InBwdObj {
     const float2* psi;   // ws_psi[b][m][s]
     float2* gobj;        // g_object + s*H*W + ry*W + rx
     template <class SH, int R>
-    PTY_DEV void load(const Cta<SH>& c, int n2, int line, int gline, float2 (&v)[R]) {
+    PTY_DEV void apply(const Cta<SH>&, int n2, int, int gline, float2 (&v)[R]) {
         using I = ShapeInfo<SH>;
         constexpr int CH = 8;
 #pragma unroll
@@ -204,7 +204,7 @@ struct InBwdObj {
 #pragma unroll
             for (int q = 0; q < CH; ++q) {
                 const int row = I::R2 * (h + q) + n2;
-                const float2 g = c.S[row * I::PITCH + line];
+                const float2 g = v[h + q];
                 red_add2(gobj + (size_t)row * W + gline, cmulc(ps[q], g));
                 v[h + q] = cmulc(o[q], g);
             }
@@ -217,14 +217,14 @@ struct InBwdProp {
     const float2* hat;   // ws_hat[b][m][s-1] or null
     float acc_ky, acc_kx, acc_k2;
     template <class SH, int R>
-    PTY_DEV void load(const Cta<SH>& c, int n2, int line, int gline, float2 (&v)[R]) {
+    PTY_DEV void apply(const Cta<SH>& c, int n2, int, int gline, float2 (&v)[R]) {
         using I = ShapeInfo<SH>;
         const float2 myl = c.My[gline];
         const float kyl = kp_of<I::N>(gline);
 #pragma unroll
         for (int n1 = 0; n1 < R; ++n1) {
             const int row = I::R2 * n1 + n2;
-            const float2 g = c.S[row * I::PITCH + line];
+            const float2 g = v[n1];
             if (hat) {
                 const float2 hs = ld_stream2(hat + row * I::N + gline);
                 const float d = hs.x * g.y - hs.y * g.x;       // Im(conj(psi^) g^)
@@ -268,17 +268,18 @@ PTY_DEV void fwd_body(const KArgs& A, const Cta<SH>& c, int item) {
     setup_tables(c, A, b, ry, rx);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)item;
-    {   // psi_0 = F^-1[E . P^]
+    {   // psi_0 = F^-1[E . P^] (up to the last stage B: the object multiply of slice 0 is fused into it)
         InProbe in{A.probe_hat + (size_t)m * NN};
-        fft_2d<SH, +1>(c, in);
+        fft_begin<SH, +1>(c, in);
     }
     for (int s = 0; s < A.Nz; ++s) {
         InFwdObj in{A.object + obj_off + ((size_t)s * A.H + ry) * A.W + rx, A.W, A.ws_psi + (bm * A.Nz + s) * NN};
-        fft_2d<SH, -1>(c, in);
+        fft_link<SH, +1, -1>(c, in);
         if (s == A.Nz - 1) break;
         InFwdProp ip{A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + s) * NN : nullptr};
-        fft_2d<SH, +1>(c, ip);
+        fft_link<SH, -1, +1>(c, ip);
     }
+    fft_end<SH, -1>(c);
     // a5: Psi = F[phi_Nz] (unitary), I += |Psi|^2; both in the transposed k-space order [k_x][k_y]
     float2* Psi = A.ws_Psi + bm * NN;
     float* Ib = A.I + (size_t)b * NN;
@@ -306,17 +307,18 @@ PTY_DEV void bwd_body(const KArgs& A, const Cta<SH>& c, int item) {
     const size_t bm = (size_t)item;
     {   // B1, B2
         InSeed in{A.ws_Psi + bm * NN, A.seed_w + (size_t)b * NN};
-        fft_2d<SH, +1>(c, in);
+        fft_begin<SH, +1>(c, in);
     }
     InBwdProp ip{nullptr, 0.f, 0.f, 0.f};
     for (int s = A.Nz - 1; s >= 0; --s) {
         const size_t off = obj_off + ((size_t)s * A.H + ry) * A.W + rx;
         InBwdObj in{A.object + off, A.W, A.ws_psi + (bm * A.Nz + s) * NN, A.g_object + off};
-        fft_2d<SH, -1>(c, in);
+        fft_link<SH, +1, -1>(c, in);
         if (s == 0) break;
         ip.hat = A.save_hat ? A.ws_hat + (bm * (A.Nz - 1) + (s - 1)) * NN : nullptr;
-        fft_2d<SH, +1>(c, ip);
+        fft_link<SH, -1, +1>(c, ip);
     }
+    fft_end<SH, -1>(c);
     // B6, B7: g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
     const float2* Ph = A.probe_hat + (size_t)m * NN;
     float2* GP = A.GP_hat + (size_t)m * NN;
