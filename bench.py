@@ -256,6 +256,7 @@ def main():
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="replay each step (forward + gradient of one minibatch) as one CUDA graph; auto = on for the "
                          "launch-bound small configurations 1 and 2 on one GPU")
+    ap.add_argument("--e2e-plans", type=int, default=3, help="plans / streams of the pipelined end-to-end measurement")
     ap.add_argument("--plan-flags", type=int, default=0,
                     help="extra pty_dims.flags for the timed plan (16 = PTY_FLAG_TMA_OBJECT, 32 = PTY_FLAG_PAIR_SUM): "
                          "opt-in kernel variants, reported in config.plan_flags")
@@ -405,34 +406,38 @@ def main():
         # The same call without its final synchronisation (pty_grad_host_async / pty_grad_host_wait), two plans on two
         # streams fed alternately: the copies of one minibatch overlap the kernels of the other.  Every step still
         # copies all of its inputs host -> device and all of its results device -> host.
-        plan2 = binding.plan_for(cfg, Bmax=B, flags=binding.PTY_FLAG_HOST | args.plan_flags, device=local)
-        plans, streams = [plan, plan2], [torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)]
-        outs = [(h_loss, h_go, h_gp, h_gq, h_gt),
-                (torch.zeros(1, dtype=torch.float64).pin_memory(), torch.zeros_like(h_obj).pin_memory(),
-                 torch.zeros_like(h_probe).pin_memory(), torch.zeros(B, 2).pin_memory(),
-                 torch.zeros(2).pin_memory() if tilt is not None else None)]
+        NP = max(2, args.e2e_plans)
+        plans = [plan] + [binding.plan_for(cfg, Bmax=B, flags=binding.PTY_FLAG_HOST | args.plan_flags, device=local)
+                          for _ in range(NP - 1)]
+        streams = [torch.cuda.Stream(device=dev) for _ in range(NP)]
+        outs = [(h_loss, h_go, h_gp, h_gq, h_gt)] + [
+            (torch.zeros(1, dtype=torch.float64).pin_memory(), torch.zeros_like(h_obj).pin_memory(),
+             torch.zeros_like(h_probe).pin_memory(), torch.zeros(B, 2).pin_memory(),
+             torch.zeros(2).pin_memory() if tilt is not None else None) for _ in range(NP - 1)]
 
         def enqueue(i):
-            k = i & 1
+            k = i % NP
             with torch.cuda.stream(streams[k]):
                 plans[k].grad_host(h_obj, h_probe, h_pos[i % len(h_pos)], h_tilt, h_meas[i % len(h_meas)], *outs[k],
                                    wait=False)
 
-        k_pipe = 2 * max(2, min(args.steps, 8) // 2)
-        for i in range(2):
+        k_pipe = NP * max(2, min(args.steps, 8) // 2)
+        for i in range(NP):
             enqueue(i)
             plans[i].grad_host_wait()
         barrier()
         t0 = time.perf_counter()
         for i in range(k_pipe):
+            if i >= NP:
+                plans[i % NP].grad_host_wait()        # the step that used this plan NP steps ago
             enqueue(i)
-            if i > 0:
-                plans[(i - 1) & 1].grad_host_wait()
-        plans[(k_pipe - 1) & 1].grad_host_wait()
+        for k in range(NP):
+            plans[k].grad_host_wait()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        pipe_loss = float(outs[(k_pipe - 1) & 1][0].item())
-        plan2.close()
+        pipe_loss = float(outs[(k_pipe - 1) % NP][0].item())
+        for q in plans[1:]:
+            q.close()
         if world > 1:
             t = torch.tensor([dt, dt_serial], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -441,8 +446,8 @@ def main():
         d2h = 8 + h_go.numel() * 8 + h_gp.numel() * 8 + B * 8 + (8 if tilt is not None else 0)
         e2e = {"value": world * B * k_pipe / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": k_pipe,
-               "api": "pty_grad_host_async + pty_grad_host_wait (pinned host buffers; two plans on two streams, the "
-                      "copies of one minibatch overlap the kernels of the other)",
+               "api": f"pty_grad_host_async + pty_grad_host_wait (pinned host buffers; {NP} plans on {NP} streams fed in "
+                      "turn: the copies of one minibatch overlap the kernels of another)",
                "loss": pipe_loss,
                "serial": {"value": world * B * k_e2e / dt_serial, "steps": k_e2e, "loss": serial_loss,
                           "api": "pty_grad_host, one call after the other"}}
