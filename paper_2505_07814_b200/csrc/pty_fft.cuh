@@ -23,6 +23,9 @@
 #ifndef PTY_STAGE_A_UNROLL
 #define PTY_STAGE_A_UNROLL 1   // both tasks of a thread in flight in stage A (c5: +2 %)
 #endif
+#ifndef PTY_DSMEM_ASYNC
+#define PTY_DSMEM_ASYNC 1
+#endif
 #ifndef PTY_CLUSTER_RELAXED
 #define PTY_CLUSTER_RELAXED 1   // N = 256: the write-after-read cluster barrier of stage B arrives without a release fence (c5: 22.9 -> 22.2 ms)
 #endif
@@ -171,7 +174,8 @@ template <class SH> struct ShapeInfo {
     static constexpr size_t table_bytes = size_t(5) * N * sizeof(float2) + 64 * sizeof(float);
     // cluster shapes: two staging tiles NL x (NL + 1) for the coalesced DSMEM transpose (stage_b)
     static constexpr size_t stage_bytes = CL > 1 ? size_t(2) * NL * (NL + 1) * sizeof(float2) : 0;
-    static constexpr size_t smem_bytes = wave_bytes + table_bytes + stage_bytes;
+    // cluster shapes: + the mbarrier that counts the bytes arriving from the peers (st.async exchange)
+    static constexpr size_t smem_bytes = wave_bytes + table_bytes + stage_bytes + (CL > 1 ? 16 : 0);
 };
 
 // Per-CTA view: thread id, rank in the cluster, the wave buffer of every CTA of the cluster
@@ -183,6 +187,8 @@ template <class SH> struct Cta {
     float2 *tw, *Ey, *Ex, *My, *Mx;   // [N] each: twiddles exp(-2 pi i j/N); shift and propagator factors
     float* red;                       // [64] block-reduction scratch
     float2* stg;                      // cluster shapes: 2 staging tiles [NL][NL + 1]
+    unsigned long long* rx;           // cluster shapes: mbarrier completed by the peers' st.async of one exchange
+    mutable unsigned rx_phase;        // parity of the exchange this CTA waits for next
 };
 
 template <class SH> PTY_DEV void sync_all() {
@@ -266,6 +272,10 @@ PTY_DEV void stage_b_exchange(const Cta<SH>& c, float2 (&v)[ShapeInfo<SH>::TB][S
         unsigned rbase;
         asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbase)
                      : "r"((unsigned)__cvta_generic_to_shared(c.S + (size_t)(RANK * I::NL) * I::PITCH)), "r"(d));
+#if PTY_DSMEM_ASYNC
+        unsigned rbar;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbar) : "r"((unsigned)__cvta_generic_to_shared(c.rx)), "r"(d));
+#endif
         float2 tv[(I::NL * I::NL) / I::NT];
 #pragma unroll
         for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
@@ -276,7 +286,14 @@ PTY_DEV void stage_b_exchange(const Cta<SH>& c, float2 (&v)[ShapeInfo<SH>::TB][S
         for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
             const int idx = j * I::NT + c.tid;
             const unsigned a = rbase + (unsigned)(((idx / I::NL) * I::PITCH + idx % I::NL) * sizeof(float2));
+#if PTY_DSMEM_ASYNC
+            // asynchronous remote store: its 8 bytes are counted on the RECEIVER's mbarrier, so the exchange needs neither
+            // a release fence (which would also drain this thread's saved-wave stores to HBM) nor a closing cluster barrier
+            asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
+                         ::"r"(a), "f"(tv[j].x), "f"(tv[j].y), "r"(rbar) : "memory");
+#else
             asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(tv[j].x), "f"(tv[j].y) : "memory");
+#endif
         }
     }
 }
@@ -328,12 +345,22 @@ PTY_DEV void stage_b(const Cta<SH>& c) {
         // per destination; destinations start at the own rank so that the four CTAs do not target one peer.
         // The rank is a template parameter of the exchange (a CTA-uniform switch), so the destination of every register
         // is known at compile time: no predicated-off stores, and the tile for the own CTA is written in place.
+#if PTY_DSMEM_ASYNC
+        // this CTA expects the tiles of its CL - 1 peers (one arrival: this post; the bytes: their st.async)
+        if (c.tid == 0) mbar_expect_tx(c.rx, (unsigned)((SH::CL - 1) * I::NL * I::NL * sizeof(float2)));
+#endif
         switch (c.rank) {
             case 0: stage_b_exchange<SH, 0>(c, v); break;
             case 1: stage_b_exchange<SH, 1 % SH::CL>(c, v); break;
             case 2: stage_b_exchange<SH, 2 % SH::CL>(c, v); break;
             default: stage_b_exchange<SH, 3 % SH::CL>(c, v); break;
         }
+#if PTY_DSMEM_ASYNC
+        mbar_wait(c.rx, c.rx_phase);      // every peer's tile has landed in this CTA's wave
+        c.rx_phase ^= 1u;
+        pty_cta_sync();                   // ... and this CTA's own tile (written in place by its threads)
+        return;
+#endif
     }
     sync_all<SH>();
 }

@@ -39,6 +39,11 @@ __device__ __forceinline__ Cta<SH> make_cta(unsigned char* smem) {
     c.tw = tab; c.Ey = tab + SH::N; c.Ex = tab + 2 * SH::N; c.My = tab + 3 * SH::N; c.Mx = tab + 4 * SH::N;
     c.red = reinterpret_cast<float*>(tab + 5 * SH::N);
     c.stg = reinterpret_cast<float2*>(smem + I::wave_bytes + I::table_bytes);
+    c.rx = reinterpret_cast<unsigned long long*>(smem + I::wave_bytes + I::table_bytes + I::stage_bytes);
+    c.rx_phase = 0;
+    if constexpr (SH::CL > 1) {     // made visible to the peers by the cluster barrier that follows make_cta in the kernels
+        if (threadIdx.x == 0) { mbar_init(c.rx, 1); mbar_init_fence(); }
+    }
     return c;
 }
 
