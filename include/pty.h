@@ -261,6 +261,44 @@ int pty_grad_host_async(pty_plan* plan, const void* h_object, const void* h_prob
                   float* h_g_tilt, void* stream);
 int pty_grad_host_wait(pty_plan* plan);
 
+/* Probe-mode orthogonalisation for callers that have no device memory to give (the same operation
+ * as pty_constrain with ortho_probe = 1, the same three kernels, the same results).
+ *
+ * Who needs it.  Every other entry point takes a plan, and a plan lives in a device workspace that the CALLER has to
+ * allocate.  Some callers cannot: a host application that handed the whole device to its own memory pool when it
+ * started (any further cudaMalloc fails, and the pool hands nothing to plug-ins), a plug-in or post-processing hook
+ * that is given the probe pointer and a stream and nothing else, or a control loop that may not stall -- cudaMalloc
+ * and cudaFree synchronise the device.  Such a caller still wants the probe modes orthogonalised between iterations.
+ *
+ * How.  No plan, no workspace, and the call makes no cudaMalloc, cudaFree or other allocating call.  The scratch
+ * the operation needs (Gram matrix, eigenvectors, eigenvalues: 33,024 bytes) is a fixed array inside libpty.so's
+ * device image, sized for the limit below; every GPU on which the library's kernels get loaded holds those 33 KB
+ * until the process exits, whether or not this function is ever called.
+ *
+ *   probe   [M][N][N] c64 on `device`, 8-byte aligned; replaced in place by the orthogonal modes of the same
+ *           mixed state, ordered by decreasing power
+ *   M       1 .. PTY_ORTHO_NOALLOC_MAX_MODES; more modes do not fit the fixed scratch: PTY_ERR_UNSUPPORTED, and the
+ *           text from pty_last_error(NULL) names the limit (use pty_constrain with a plan for larger M -- which
+ *           has the same limit today)
+ *   N       1 .. 4096 (any window size, not only 64 / 128 / 256)
+ *   device  CUDA device ordinal that owns `probe`; made current for the call, the caller's device is restored
+ *   stream  a stream of that device; the three kernels are enqueued on it and the call does not synchronise
+ *
+ * First call on a device.  It looks up the device address of the scratch array (cudaGetSymbolAddress, which may
+ * load the library's kernels onto that device) and remembers it per device.  Make that first call during start-up,
+ * outside any stream capture; later calls on that device only launch kernels.
+ *
+ * Sharing.  There is ONE scratch array per device for the whole process.  Nothing in it has to start at zero:
+ * a call overwrites every element it later reads, so the previous call's contents (which stay there) do no
+ * harm.  Two calls whose kernels can overlap on the same device -- different streams, different host threads --
+ * race on it and give wrong modes: keep all calls for one device on one stream, or order them with events.
+ *
+ * Errors: PTY_ERR_INVALID_ARG (null or misaligned probe, M < 1, N out of range, bad device), PTY_ERR_UNSUPPORTED
+ * (M beyond the limit), PTY_ERR_CUDA; the text is returned by pty_last_error(NULL) on the calling thread. */
+#define PTY_ORTHO_NOALLOC_MAX_MODES   32
+#define PTY_ORTHO_NOALLOC_SCRATCH_BYTES  (2 * 32 * 32 * 16 + 32 * 8)    /* 33,024 per GPU */
+int pty_ortho_probe_noalloc(void* probe, int32_t M, int32_t N, int device, void* stream);
+
 /* Synchronises the plan's last stream and returns PTY_OK, PTY_ERR_BOUNDS or PTY_ERR_CUDA.
  * device_flags (host, may be NULL) receives the raw sticky flag word and clears it. */
 int pty_status(pty_plan* plan, int32_t* device_flags);

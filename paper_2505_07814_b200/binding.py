@@ -30,8 +30,8 @@ EXPORTS = ["pty_workspace_bytes", "pty_create", "pty_destroy", "pty_forward_loss
            "pty_step", "pty_adam_update", "pty_grad_host", "pty_status", "pty_profile",
            "pty_profile_read", "pty_set_loss", "pty_loss_terms", "pty_forward_loss_ap", "pty_backward_ap",
            "pty_step_ap", "pty_constrain", "pty_rz_filter_object", "pty_grad_host_async", "pty_grad_host_wait",
-           "pty_launch_count", "pty_last_error", "pty_version"]
-_INT_RETURNS = EXPORTS[:20]
+           "pty_ortho_probe_noalloc", "pty_launch_count", "pty_last_error", "pty_version"]
+_INT_RETURNS = EXPORTS[:21]
 
 
 class pty_dims(C.Structure):
@@ -101,6 +101,7 @@ lib.pty_step_ap.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.POIN
                             C.POINTER(pty_adam_state_ap), _vp, _vp]
 lib.pty_constrain.argtypes = [_vp, _vp, _vp, _vp, C.POINTER(pty_constraints), _vp]
 lib.pty_rz_filter_object.argtypes = [_vp, _vp, C.c_float, _vp]
+lib.pty_ortho_probe_noalloc.argtypes = [_vp, C.c_int32, C.c_int32, C.c_int, _vp]
 for _n in _INT_RETURNS:
     getattr(lib, _n).restype = C.c_int
 
@@ -288,3 +289,22 @@ def plan_for(cfg, Bmax=None, flags=0, device=0, n_obj=1):
     """Plan for a ``synth.Config``."""
     return Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, cfg.B if Bmax is None else Bmax, cfg.dz, cfg.lam, cfg.dx,
                 tilt_mode=cfg.tilt_mode, flags=flags, device=device, n_obj=n_obj)
+
+
+ORTHO_NOALLOC_MAX_MODES = 32
+
+
+def ortho_probe_noalloc(probe):
+    """pty_ortho_probe_noalloc: orthogonalise the modes of ``probe`` [M, N, N] (complex64, CUDA) in place without a
+    plan or a workspace -- for callers that have no device memory to give the library (a host application whose pool
+    already owns the whole GPU, a hook that only receives the probe).  The scratch is a fixed 33 KB array inside
+    libpty.so, one per GPU and shared by every call: M <= 32, and calls that can overlap on one GPU race, so keep them
+    on one stream.  Make the first call on each device at start-up, outside stream capture (it looks the array up).
+    Enqueued on torch's current stream of the probe's device; does not synchronise."""
+    if probe.dim() != 3 or probe.shape[1] != probe.shape[2]:
+        raise ValueError("probe must be [M, N, N]")
+    with torch.cuda.device(probe.device):
+        rc = lib.pty_ortho_probe_noalloc(_ptr(probe, torch.complex64, "cuda"), probe.shape[0], probe.shape[1],
+                                         probe.device.index, _stream())
+    if rc != PTY_OK:
+        raise PtyError(rc, lib.pty_last_error(None).decode())

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -738,6 +739,36 @@ int adam_launch(pty_plan* p, float* theta, const float* g, float* m, float* v, s
 
 }  // namespace
 
+// ---------------------------------------------------------------------------- scratch of pty_ortho_probe_noalloc
+// The one piece of device memory this library owns: Gram matrix, eigenvectors and eigenvalues of the probe-mode
+// orthogonalisation for callers that cannot hand over a workspace (include/pty.h).  It is part of the module's
+// device image, so every GPU that loads the module holds these 33,024 bytes until the process exits.
+// In HOST code the name below is only a handle for the runtime's symbol calls, not a device address: handing it to a
+// kernel would make the kernel fault, or, where the GPU can reach host memory, read and write the wrong memory without
+// a fault.  noalloc_scratch() asks the runtime for the real address on each device and only that goes to the kernels.
+static_assert(PTY_ORTHO_NOALLOC_MAX_MODES == pty::kMaxModes, "pty.h and the eigen-solver disagree on the mode limit");
+static __device__ __align__(256) unsigned char g_ortho_noalloc_scratch[PTY_ORTHO_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+unsigned char* g_noalloc_addr[kNoAllocMaxDevices];      // device address of the array on device i; null = not asked yet
+
+// Address of the scratch array on `device`, which the caller has made current.  The first call per device asks the
+// runtime (this is the set-up step pty.h tells callers to run before any stream capture); later calls read the table.
+int noalloc_scratch(int device, unsigned char** out) {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[device]) {
+        unsigned char* ptr = nullptr;
+        PTY_CUDA(nullptr, cudaGetSymbolAddress((void**)&ptr, g_ortho_noalloc_scratch));
+        if (!ptr) return fail(nullptr, PTY_ERR_CUDA, "cudaGetSymbolAddress returned a null scratch address on device %d", device);
+        g_noalloc_addr[device] = ptr;
+    }
+    *out = g_noalloc_addr[device];
+    return PTY_OK;
+}
+}  // namespace
+
 // ============================================================================ C ABI
 extern "C" {
 
@@ -1216,6 +1247,43 @@ int pty_rz_filter_object(pty_plan* plan, void* object, float sigma_z, void* stre
     // complex64 = interleaved (re, im): a plane of H W complex values is 2 H W floats
     return rz_filter_launch(plan, static_cast<float*>(object), (size_t)plan->n_obj(), (size_t)plan->d.H * plan->d.W * 2, sigma_z,
                             static_cast<cudaStream_t>(stream));
+}
+
+// Probe-mode orthogonalisation without a plan, a workspace or any allocation (include/pty.h): the three kernels of
+// pty_constrain's ortho_probe branch, with their scratch in the library's own static device array.
+int pty_ortho_probe_noalloc(void* probe, int32_t M, int32_t N, int device, void* stream) {
+    if (!probe) return fail(nullptr, PTY_ERR_INVALID_ARG, "pty_ortho_probe_noalloc: probe is null");
+    if (reinterpret_cast<uintptr_t>(probe) % 8) return fail(nullptr, PTY_ERR_INVALID_ARG, "pty_ortho_probe_noalloc: probe must be 8-byte aligned");
+    if (M < 1) return fail(nullptr, PTY_ERR_INVALID_ARG, "pty_ortho_probe_noalloc: M = %d, need at least one mode", (int)M);
+    if (M > PTY_ORTHO_NOALLOC_MAX_MODES)
+        return fail(nullptr, PTY_ERR_UNSUPPORTED, "pty_ortho_probe_noalloc: M = %d modes do not fit the fixed %d-byte scratch (limit: %d modes)",
+                    (int)M, (int)PTY_ORTHO_NOALLOC_SCRATCH_BYTES, (int)PTY_ORTHO_NOALLOC_MAX_MODES);
+    if (N < 1 || N > 4096) return fail(nullptr, PTY_ERR_INVALID_ARG, "pty_ortho_probe_noalloc: N = %d, need 1 <= N <= 4096", (int)N);
+    if (device < 0 || device >= kNoAllocMaxDevices)
+        return fail(nullptr, PTY_ERR_INVALID_ARG, "pty_ortho_probe_noalloc: device %d outside [0, %d)", device, kNoAllocMaxDevices);
+    DeviceGuard dg(device);
+    int current = -1;
+    PTY_CUDA(nullptr, cudaGetDevice(&current));
+    if (current != device) return fail(nullptr, PTY_ERR_INVALID_ARG, "pty_ortho_probe_noalloc: cannot make device %d current", device);
+    unsigned char* scratch = nullptr;
+    int rc;
+    if ((rc = noalloc_scratch(device, &scratch))) return rc;
+    // the workspace layout of the plan path (make_layout: gram, eigv, eigl), at its largest M
+    constexpr size_t kMat = (size_t)PTY_ORTHO_NOALLOC_MAX_MODES * PTY_ORTHO_NOALLOC_MAX_MODES * sizeof(double2);
+    double2* G = reinterpret_cast<double2*>(scratch);
+    double2* V = reinterpret_cast<double2*>(scratch + kMat);
+    double* lam = reinterpret_cast<double*>(scratch + 2 * kMat);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t NN = (size_t)N * N;
+    const size_t blocks = std::min<size_t>((NN + 255) / 256, 148 * 16);
+    // every G, V, lam element read below is written first by the kernel before it: nothing needs clearing between calls
+    pty_gram_kernel<<<M * (M + 1) / 2, 256, 0, st>>>((const float2*)probe, (int)M, NN, G);
+    PTY_CUDA(nullptr, cudaGetLastError());
+    pty_eigh_kernel<<<1, 32, 0, st>>>((const double2*)G, (int)M, V, lam);
+    PTY_CUDA(nullptr, cudaGetLastError());
+    pty_mix_modes_kernel<<<(unsigned)blocks, 256, 0, st>>>((float2*)probe, (int)M, NN, (const double2*)V);
+    PTY_CUDA(nullptr, cudaGetLastError());
+    return PTY_OK;
 }
 
 int pty_status(pty_plan* plan, int32_t* device_flags) {
