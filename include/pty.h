@@ -62,6 +62,9 @@ extern "C" {
 #define PTY_ERR_WORKSPACE     (-3)  /* workspace null, misaligned (256 B) or too small        */
 #define PTY_ERR_CUDA          (-4)  /* a CUDA runtime call failed; see pty_last_error         */
 #define PTY_ERR_BOUNDS        (-5)  /* pty_status: some crop left the object and was clamped  */
+#define PTY_ERR_ZERO_DATA     (-6)  /* pty_status: a loss-mode-1 call saw a minibatch whose measurements are all
+                                       zero; Eq. 5-7 divide by their mean, so the affected terms and their
+                                       gradients were set to 0 instead of inf / NaN (sticky flag bit 2)      */
 
 /* pty_dims.flags */
 #define PTY_FLAG_SPECTRA       1    /* keep propagated spectra so that g_dz can be produced even
@@ -80,9 +83,9 @@ extern "C" {
                                        probe modes a CTA holds (two groups, one position) in a shared-memory
                                        ring before the one global reduction per pixel -- the on-chip part of
                                        the crop's adjoint: half the atomics,
-                                       same results up to the summation order.  Needs an even n_obj * M
-                                       (otherwise a CTA's two items can belong to two positions and the
-                                       per-item reductions run).  Off by default: the ring couples the two
+                                       same results up to the summation order.  Needs an even M
+                                       (otherwise a CTA's two items can belong to two positions or two object
+                                       states and the per-item reductions run).  Off by default: the ring couples the two
                                        groups' phases and is measured slower      */
 
 /* pty_backward flags */
@@ -299,7 +302,8 @@ int pty_grad_host_wait(pty_plan* plan);
 #define PTY_ORTHO_NOALLOC_SCRATCH_BYTES  (2 * 32 * 32 * 16 + 32 * 8)    /* 33,024 per GPU */
 int pty_ortho_probe_noalloc(void* probe, int32_t M, int32_t N, int device, void* stream);
 
-/* Synchronises the plan's last stream and returns PTY_OK, PTY_ERR_BOUNDS or PTY_ERR_CUDA.
+/* Synchronises the plan's last stream and returns PTY_OK, PTY_ERR_BOUNDS (flag bit 1; wins if both are set),
+ * PTY_ERR_ZERO_DATA (flag bit 2) or PTY_ERR_CUDA.
  * device_flags (host, may be NULL) receives the raw sticky flag word and clears it. */
 int pty_status(pty_plan* plan, int32_t* device_flags);
 

@@ -22,7 +22,7 @@ if not os.path.exists(LIB_PATH):
 lib = C.CDLL(LIB_PATH)
 
 PTY_OK, PTY_ERR_INVALID_ARG, PTY_ERR_UNSUPPORTED = 0, -1, -2
-PTY_ERR_WORKSPACE, PTY_ERR_CUDA, PTY_ERR_BOUNDS = -3, -4, -5
+PTY_ERR_WORKSPACE, PTY_ERR_CUDA, PTY_ERR_BOUNDS, PTY_ERR_ZERO_DATA = -3, -4, -5, -6
 PTY_FLAG_SPECTRA, PTY_FLAG_STEP, PTY_FLAG_HOST, PTY_FLAG_AMP_PHASE, PTY_FLAG_TMA_OBJECT, PTY_FLAG_PAIR_SUM = 1, 2, 4, 8, 16, 32
 PTY_BWD_ACCUMULATE, PTY_BWD_REUSE_FORWARD = 1, 4
 

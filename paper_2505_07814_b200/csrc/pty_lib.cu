@@ -123,7 +123,8 @@ __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A
     release_g2(smem);
 }
 // PAIR: the two groups of a CTA sum their g_object contributions in shared memory before the one reduction (G2Pair;
-// the host selects it only when every item pair 2x, 2x + 1 holds two modes of one position, i.e. n_obj M is even)
+// the host selects it only when every item pair 2x, 2x + 1 holds two modes of one position AND one object state,
+// i.e. M is even: with an odd M and an even n_obj a pair would span two states, whose gradients are separate arrays)
 template <bool HAT, bool PAIR> __global__ void __launch_bounds__(F128::NT, 1) pty_bwd128g2_kernel(const KArgs A) {
     extern __shared__ __align__(128) unsigned char smem[];
     const G2 c = make_g2(smem);
@@ -566,7 +567,7 @@ cudaError_t launch_bwd(pty_plan* p, const KArgs& A, cudaStream_t st) {
     ScopedTimer tm(p, 1, st);
     if (p->d.N == 128)
     {
-        if ((p->d.flags & PTY_FLAG_PAIR_SUM) && A.MT % 2 == 0)
+        if ((p->d.flags & PTY_FLAG_PAIR_SUM) && A.M % 2 == 0)    // item = (b n_obj + n) M + m: an even M keeps a pair in one (b, n)
             return A.save_hat ? launch(p, pty_bwd128g2_kernel<true, true>, g2_grid(p, A), F128::NT, G2Pair::bytes, 1, st, A)
                               : launch(p, pty_bwd128g2_kernel<false, true>, g2_grid(p, A), F128::NT, G2Pair::bytes, 1, st, A);
         return A.save_hat ? launch(p, pty_bwd128g2_kernel<true, false>, g2_grid(p, A), F128::NT, G2Smem::bytes, 1, st, A)
@@ -630,18 +631,25 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
     const size_t NN = (size_t)d.N * d.N;
     p->last_stream = st;
     p->fwd_valid = false;
+    // one-shot hand-overs from ap_prepare / pty_grad_host: taken and cleared here so that no exit path (B == 0, a CUDA
+    // error) leaves them set for the next, unrelated call on this plan
+    const bool sparse_ready = p->sparse_ready, wait_meas = p->wait_meas;
+    p->sparse_ready = false;
+    p->wait_meas = false;
     PTY_CUDA(p, cudaMemsetAsync(loss, 0, sizeof(double), st));
-    if (B == 0) return PTY_OK;
+    if (B == 0) {
+        if (wait_meas) PTY_CUDA(p, cudaStreamWaitEvent(st, p->ev_meas, 0));
+        return PTY_OK;
+    }
     const bool paper_loss = p->loss_cfg.mode == 1;
     if (paper_loss) {   // the minibatch sums of Eq. 5-7 (the AP entry point has already put L_sparse in place)
-        if (!p->sparse_ready) PTY_CUDA(p, cudaMemsetAsync(p->d_stats(), 0, ST_COUNT * sizeof(double), st));
+        if (!sparse_ready) PTY_CUDA(p, cudaMemsetAsync(p->d_stats(), 0, ST_COUNT * sizeof(double), st));
         else PTY_CUDA(p, cudaMemsetAsync(p->d_stats(), 0, 4 * sizeof(double), st));
         if (p->loss_cfg.w_pacbed != 0.f) {
             PTY_CUDA(p, cudaMemsetAsync(p->at<float>(p->L.Isum), 0, NN * sizeof(float), st));
             PTY_CUDA(p, cudaMemsetAsync(p->at<float>(p->L.Imsum), 0, NN * sizeof(float), st));
         }
     }
-    p->sparse_ready = false;
     KArgs A = make_args(p, object, positions, tilt, meas, B);
     // a0: probe spectrum (unitary) and propagator factors
     if (d.N == 128)
@@ -653,21 +661,19 @@ int run_forward(pty_plan* p, const void* object, const void* probe, const float*
                            d.tilt_mode == 1 ? tilt : (const float*)nullptr, p->at<float2>(p->L.prop), p->at<float2>(p->L.prop) + d.N));
     PTY_CUDA(p, cudaMemsetAsync(A.I, 0, (size_t)B * NN * sizeof(float), st));
     PTY_CUDA(p, launch_fwd(p, A, st));
-    if (p->wait_meas) {      // pty_grad_host: the loss is the first reader of the measurements
-        p->wait_meas = false;
+    if (wait_meas)           // pty_grad_host: the loss is the first reader of the measurements
         PTY_CUDA(p, cudaStreamWaitEvent(st, p->ev_meas, 0));
-    }
     if (paper_loss) {
         const LossCfg cfg = p->loss_dev();
         float* Isum = p->at<float>(p->L.Isum);
         float* Imsum = p->at<float>(p->L.Imsum);
         if (d.N == 128) {
             PTY_CUDA(p, launch(p, pty_loss_sums_kernel<true>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, cfg, p->d_stats(), loss_per_pos, Isum, Imsum, intensity));
-            PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss));
+            PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss, p->d_flags()));
             PTY_CUDA(p, launch(p, pty_seed_kernel<true>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, (int)B, cfg, (const double*)p->d_stats(), (const float*)Isum, (const float*)Imsum, A.seed_w));
         } else {
             PTY_CUDA(p, launch(p, pty_loss_sums_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, cfg, p->d_stats(), loss_per_pos, Isum, Imsum, intensity));
-            PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss));
+            PTY_CUDA(p, launch(p, pty_loss_finalize_kernel, 1, 256, 0, 1, st, (int)B, (int)d.N, cfg, p->d_stats(), (const float*)Isum, (const float*)Imsum, loss, p->d_flags()));
             PTY_CUDA(p, launch(p, pty_seed_kernel<false>, B, 256, 0, 1, st, (const float*)A.I, meas, (int)d.N, (int)B, cfg, (const double*)p->d_stats(), (const float*)Isum, (const float*)Imsum, A.seed_w));
         }
     } else if (d.N == 128) {
@@ -1296,6 +1302,7 @@ int pty_status(pty_plan* plan, int32_t* device_flags) {
     if (device_flags) *device_flags = flags;
     PTY_CUDA(plan, cudaGetLastError());
     if (flags & 1) return fail(plan, PTY_ERR_BOUNDS, "a scan position's crop left the object and was clamped");
+    if (flags & 2) return fail(plan, PTY_ERR_ZERO_DATA, "loss mode 1 on a minibatch of all-zero measurements: the normalised terms were set to 0");
     return PTY_OK;
 }
 

@@ -123,8 +123,10 @@ __global__ void __launch_bounds__(256) pty_loss_sums_kernel(const float* __restr
 
 // Eq. 5-7 + Eq. 9, pass 2 (one block): the normalised terms, the total, and the coefficients of dL/dI:
 //   dL/dI_b(k) = cG (1 - a / sqrt(I)) + cP (1 - a^2 / (I + eps)) + cPB (1 - sqrt(<I_meas>_B / <I>_B)).
+// A minibatch whose measurements are all zero has no mean to normalise by (Eq. 5-7 divide by <a> and <a^2>): the terms
+// and coefficients that would divide by zero are set to 0 and sticky flag bit 2 is raised (pty_status: PTY_ERR_ZERO_DATA).
 __global__ void __launch_bounds__(256) pty_loss_finalize_kernel(int B, int N, LossCfg cfg, double* stats, const float* Isum,
-                                                               const float* Imsum, double* loss) {
+                                                               const float* Imsum, double* loss, int* flags) {
     __shared__ double part[8];
     const double n = (double)B * N * N, nD = (double)N * N;
     double q = 0.0;
@@ -136,11 +138,14 @@ __global__ void __launch_bounds__(256) pty_loss_finalize_kernel(int B, int N, Lo
     const double Q = block_sum_256(q, part);
     if (threadIdx.x != 0) return;
     const double mean_a = stats[ST_A] / n, mse = stats[ST_S] / n, mean_im = stats[ST_A2] / n, mse_pb = Q / nD;
-    const double LG = sqrt(mse) / mean_a, LP = -(stats[ST_P] / n) / mean_im, LPB = sqrt(mse_pb) / mean_a;
+    const bool ok_a = mean_a != 0.0, ok_im = mean_im != 0.0;
+    if (!ok_a || !ok_im) atomicOr(flags, 2);
+    const double LG = ok_a ? sqrt(mse) / mean_a : 0.0, LP = ok_im ? -(stats[ST_P] / n) / mean_im : 0.0,
+                 LPB = ok_a ? sqrt(mse_pb) / mean_a : 0.0;
     stats[ST_LG] = LG; stats[ST_LP] = LP; stats[ST_LPB] = LPB;
-    stats[ST_CG] = (cfg.w_gaussian != 0.f && mse > 0.0) ? cfg.w_gaussian / (2.0 * sqrt(mse) * mean_a * n) : 0.0;
-    stats[ST_CP] = cfg.w_poisson != 0.f ? cfg.w_poisson / (n * mean_im) : 0.0;
-    stats[ST_CPB] = (cfg.w_pacbed != 0.f && mse_pb > 0.0) ? cfg.w_pacbed / (2.0 * sqrt(mse_pb) * mean_a * nD * B) : 0.0;
+    stats[ST_CG] = (cfg.w_gaussian != 0.f && mse > 0.0 && ok_a) ? cfg.w_gaussian / (2.0 * sqrt(mse) * mean_a * n) : 0.0;
+    stats[ST_CP] = (cfg.w_poisson != 0.f && ok_im) ? cfg.w_poisson / (n * mean_im) : 0.0;
+    stats[ST_CPB] = (cfg.w_pacbed != 0.f && mse_pb > 0.0 && ok_a) ? cfg.w_pacbed / (2.0 * sqrt(mse_pb) * mean_a * nD * B) : 0.0;
     *loss = cfg.w_gaussian * LG + cfg.w_poisson * LP + cfg.w_pacbed * LPB + cfg.w_sparse * stats[ST_LS];
 }
 
