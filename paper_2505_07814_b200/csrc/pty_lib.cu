@@ -1191,19 +1191,15 @@ int rz_filter_launch(pty_plan* p, float* x, size_t outer, size_t plane, float si
     if (!(sigma_z > 0.f) || Nz < 2) return PTY_OK;
     const int R = std::max(1, (int)std::ceil(2.0 * (double)sigma_z));
     if (R > 8) return fail(p, PTY_ERR_UNSUPPORTED, "r_z filter: sigma_z = %g needs a radius of %d slices (max 8)", (double)sigma_z, R);
-    float taps[17];
+    RzTaps taps{};           // by value into the launch: nothing on the host has to outlive this call (stream capture)
     double sum = 0.0;
     for (int j = -R; j <= R; ++j) sum += std::exp(-(double)j * j / (2.0 * (double)sigma_z * sigma_z));
-    for (int j = -R; j <= R; ++j) taps[j + R] = (float)(std::exp(-(double)j * j / (2.0 * (double)sigma_z * sigma_z)) / sum);
-    float* dtaps = p->at<float>(p->L.taps);
-    // the taps travel as kernel-parameter-sized data through a stream-ordered copy from a pageable host buffer
-    // (copied by the driver before the call returns)
-    PTY_CUDA(p, cudaMemcpyAsync(dtaps, taps, (2 * R + 1) * sizeof(float), cudaMemcpyHostToDevice, st));
+    for (int j = -R; j <= R; ++j) taps.t[j + R] = (float)(std::exp(-(double)j * j / (2.0 * (double)sigma_z * sigma_z)) / sum);
     const size_t columns = outer * plane;
     const int grid = grid_for(p, columns);
     cudaError_t e = cudaSuccess;
     switch (R) {
-#define PTY_RZ(RR) case RR: e = launch(p, pty_rz_filter_kernel<RR>, grid, 256, 0, 1, st, x, Nz, plane, columns, (const float*)dtaps); break;
+#define PTY_RZ(RR) case RR: e = launch(p, pty_rz_filter_kernel<RR>, grid, 256, 0, 1, st, x, Nz, plane, columns, taps); break;
         PTY_RZ(1) PTY_RZ(2) PTY_RZ(3) PTY_RZ(4) PTY_RZ(5) PTY_RZ(6) PTY_RZ(7) PTY_RZ(8)
 #undef PTY_RZ
     }

@@ -60,6 +60,10 @@ PTY_DEV void sweep_position(const float* __restrict__ Ib, const float* __restric
     } else {
         // N = 64 / 256: I and the seed weights are in the transposed k-space order [k_x][k_y] of the shared-memory-pass
         // kernels (pty_fft.cuh, fft_2d); the measured amplitudes are natural, [k_y][k_x]
+        // A direct walk of the natural index: I is read and the weights are written at a stride of N floats (one sector per
+        // lane).  Turning 32 x 32 tiles of the amplitudes through shared memory instead, so that lanes run along k_y, was
+        // measured SLOWER on c5 (round 3: 211 vs 141 us per launch, 128 blocks): with one block per position the kernel is
+        // latency-bound and the two barriers per tile cost more than the sector amplification, which L2 absorbs.
         for (int i = t; i < N * N; i += 256) {
             const int ky = i / N, kx = i - ky * N, ti = kx * N + ky;
             f(__ldg(Ib + ti), __ldg(ab + i), ti, i);
@@ -224,11 +228,14 @@ __global__ void __launch_bounds__(256) pty_amp_phase_grad_kernel(const float2* _
 // ------------------------------------------------------------------------------ constraints (NEXT-3)
 // Eq. 13: blur along depth, in place.  x is [outer][Nz][plane] floats; thread = one (outer, pixel) column, which walks
 // z keeping the 2R + 1 ORIGINAL values it needs in registers; end slices replicated (reading R31).
+// The taps travel BY VALUE as a kernel parameter: a launch (and a captured graph node) carries its own copy, so the call
+// is enqueue-only with no host buffer that has to outlive it.
+struct RzTaps { float t[17]; };
 template <int R>
-__global__ void __launch_bounds__(256) pty_rz_filter_kernel(float* x, int Nz, size_t plane, size_t columns, const float* taps) {
+__global__ void __launch_bounds__(256) pty_rz_filter_kernel(float* x, int Nz, size_t plane, size_t columns, const RzTaps taps) {
     float g[2 * R + 1];
 #pragma unroll
-    for (int j = 0; j < 2 * R + 1; ++j) g[j] = taps[j];
+    for (int j = 0; j < 2 * R + 1; ++j) g[j] = taps.t[j];
     for (size_t col = (size_t)blockIdx.x * 256 + threadIdx.x; col < columns; col += (size_t)gridDim.x * 256) {
         float* p = x + (col / plane) * (size_t)Nz * plane + col % plane;
         float win[2 * R + 1];                        // win[j] = original x[clamp(z + j - R)]

@@ -464,3 +464,73 @@ def test_all_zero_measurements_in_loss_mode_1_raise_a_flag_not_nans(pty):
                                       ol.LossWeights(1.0, 0.4, 0.6, 0.0))
     assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
     assert plan.status()[0] == 0
+
+
+def test_step_ap_and_constraints_replay_as_one_cuda_graph(pty):
+    """pty_step_ap followed by pty_constrain (r_z blur, sigma_z = 1: Eq. 13) recorded once and replayed:
+    both calls are enqueue-only (the blur's taps ride in the launch parameters, no host buffer outlives the call).
+    First replay from the initial state against the oracle's adam_step followed by rz_filter; three replays against
+    three eager rounds.  The Adam step number is a by-value argument, so a recorded graph repeats t = 1."""
+    case = CASES["c3"]()
+    cfg = case["cfg"]
+    B = len(case["positions"])
+    amp, phase = _amp_phase_of(case["object"])
+    w = ol.LossWeights(1.0, 0.0, 0.0, 0.1)
+    ref = ol.total_loss_and_gradients(None, case["probe"], case["positions"], None, case["meas"], geom_of(cfg), w, amp=amp, phase=phase)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, flags=pty.PTY_FLAG_AMP_PHASE | pty.PTY_FLAG_STEP)
+    plan.set_loss(1, w.gaussian, w.poisson, w.pacbed, w.sparse, w.eps)
+    init = {"amp": dev(amp), "phase": dev(phase), "probe": dev(case["probe"]), "positions": dev(case["positions"])}
+    cur = {k: v.clone() for k, v in init.items()}
+    meas = dev(case["meas"])
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    state = {}
+    for nm, t in cur.items():
+        n = t.numel() * (2 if t.is_complex() else 1)
+        state["m_" + nm], state["v_" + nm] = torch.zeros(n, device="cuda"), torch.zeros(n, device="cuda")
+    lr = 5e-4
+    hp = pty.pty_adam_ap(lr, lr, 1e-4, 5e-4, 0.0, 0.9, 0.999, 1e-8, 1)
+
+    def run():
+        plan.step_ap(cur["amp"], cur["phase"], cur["probe"], cur["positions"], None, meas, hp, state, loss)
+        plan.constrain(amp=cur["amp"], phase=cur["phase"], sigma_z=1.0)
+
+    def reset():
+        for k in cur:
+            cur[k].copy_(init[k])
+        for s in state.values():
+            s.zero_()
+
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    eager3 = {k: v.clone() for k, v in cur.items()}
+    reset()
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        run()
+    torch.cuda.current_stream().wait_stream(side)
+    reset()
+    with torch.cuda.graph(graph):
+        run()
+    reset()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
+    for nm, before, g in (("amp", amp, ref["g_amp"]), ("phase", phase, ref["g_phase"])):
+        stepped, _, _ = oracle.adam_step(before, g, np.zeros(before.size), np.zeros(before.size), 1, lr)
+        want = oc.rz_filter(stepped.reshape(before.shape), 1.0)
+        # |g| >> eps in the whole depth column: every tap of the blur sees a step of -lr sign(g)
+        big = np.broadcast_to(np.all(np.abs(g) > 1e-3 * np.abs(g).max(), axis=0, keepdims=True), before.shape)
+        got = cur[nm].cpu().numpy().astype(np.float64)
+        np.testing.assert_allclose(got[big], want[big], rtol=0, atol=2e-3 * lr + 4e-7)
+        assert rel_l2(got, want) <= 1e-4
+    graph.replay()
+    graph.replay()
+    torch.cuda.synchronize()
+    for nm in ("amp", "phase", "probe", "positions"):
+        a, b, z = cur[nm].cpu().numpy(), eager3[nm].cpu().numpy(), init[nm].cpu().numpy()
+        assert rel_l2(a - z, b - z) <= 2e-2, nm           # the few pixels with |g| ~ rounding may step the other way
+        assert rel_l2(a, b) <= 1e-4, nm
+    assert plan.status()[0] == 0
