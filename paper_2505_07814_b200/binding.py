@@ -13,7 +13,9 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpty.so")
+# PTY_LIB names another build of the same library (build.build_variant: a compile-time switch under test); the default
+# is the in-tree product build.  Either way a missing file is an error: there is no fallback path.
+LIB_PATH = os.environ.get("PTY_LIB") or os.path.join(_HERE, "libpty.so")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2505_07814_b200.build` "

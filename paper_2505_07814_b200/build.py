@@ -43,5 +43,20 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def build_variant(name, defines, force=False):
+    """Compile pty_lib.cu once more with extra -D switches into paper_2505_07814_b200/<name> (not part of build()):
+    used by tests that compare a compile-time switch of the kernels against the product build, e.g.
+    build_variant("libpty_strict.so", ["-DPTY_CLUSTER_RELAXED=0"]).  Load it with PTY_LIB=<path> (binding.py)."""
+    lib = os.path.join(HERE, name)
+    sources, headers = TARGETS[LIB]
+    if force or _stale(lib, sources, headers):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc] + NVCC_FLAGS + list(defines) + ["-o", lib] + [os.path.join(CSRC, s) for s in sources]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if res.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + (res.stdout + res.stderr)[-4000:])
+    return lib
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose=True))

@@ -196,6 +196,10 @@ template <class SH> PTY_DEV void sync_all() {
 }
 // Execution barrier only (write-after-read protection: every thread of the cluster has finished READING the waves into
 // registers; nothing written before it has to become visible), so the arrive carries no release fence.
+// This is an argument from how the hardware executes the barrier (a thread's earlier ld.shared have returned their data
+// before it can arrive: the values are consumed by the register transposes in between), NOT from the PTX memory model,
+// which gives a relaxed arrive no happens-before edge to the peers' later st.async.  Hence a compile-time switch
+// (PTY_CLUSTER_RELAXED = 0: the fenced barrier), and tests/test_gpu_cluster_order.py compares the bits of both builds.
 template <class SH> PTY_DEV void sync_all_war() {
 #if PTY_CLUSTER_RELAXED
     if (SH::CL > 1) {
