@@ -17,15 +17,6 @@
 #include "pty_port.cuh"
 #endif
 
-#ifndef PTY_DSMEM_PTX
-#define PTY_DSMEM_PTX 1   // N = 256: explicit st.shared::cluster for the tile copy (c5: 23.8 -> 22.9 ms forward)
-#endif
-#ifndef PTY_STAGE_A_UNROLL
-#define PTY_STAGE_A_UNROLL 1   // both tasks of a thread in flight in stage A (c5: +2 %)
-#endif
-#ifndef PTY_DSMEM_ASYNC
-#define PTY_DSMEM_ASYNC 1
-#endif
 #ifndef PTY_CLUSTER_RELAXED
 #define PTY_CLUSTER_RELAXED 1   // N = 256: the write-after-read cluster barrier of stage B arrives without a release fence (c5: 22.9 -> 22.2 ms)
 #endif
@@ -36,53 +27,16 @@ namespace pty {
 // Packed FP32x2 arithmetic (FADD2 / FMUL2 / FFMA2 on sm_100a): a complex value is one 64-bit register
 // pair, and the operand modifiers of the packed instructions (half swap, per-half negate, scalar
 // broadcast) absorb the swaps and sign changes, so every complex operation below is one or two
-// instructions.  Same FP32 lane throughput as scalar code, half the issue slots (profiles/r01_microbench.md).
-#ifndef PTY_PK_ADD
-#define PTY_PK_ADD 1
-#endif
-#ifndef PTY_PK_MUL
-#define PTY_PK_MUL 0
-#endif
-#ifndef PTY_PK_CS
-#define PTY_PK_CS 1
-#endif
-#if PTY_PK_ADD
+// instructions.  Same FP32 lane throughput as scalar code, half the issue slots (profiles/r03_fp32_pipe.md).
 PTY_DEV float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
 PTY_DEV float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
-#else
-PTY_DEV float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-PTY_DEV float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-#endif
-#if PTY_PK_MUL
-PTY_DEV float2 cmul(float2 a, float2 b) {
-    return __ffma2_rn(make_float2(a.y, a.x), make_float2(-b.y, b.y), __fmul2_rn(a, make_float2(b.x, b.x)));
-}
-// conj(a) * b
-PTY_DEV float2 cmulc(float2 a, float2 b) {
-    return __ffma2_rn(make_float2(b.y, b.x), make_float2(a.y, -a.y), __fmul2_rn(b, make_float2(a.x, a.x)));
-}
-PTY_DEV float2 cscale(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
-#else
 PTY_DEV float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 PTY_DEV float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }
 PTY_DEV float2 cscale(float2 a, float s) { return make_float2(a.x * s, a.y * s); }
-#endif
 PTY_DEV float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
-// variable twiddles of the cross-thread radix-4 stage: packed form behind its own switch (PTY_PK_TW)
-#ifndef PTY_PK_TW
-#define PTY_PK_TW 0
-#endif
-#if PTY_PK_TW
-PTY_DEV float2 cmul_tw(float2 a, float2 w) {      // a * w
-    return __ffma2_rn(make_float2(a.y, a.x), make_float2(-w.y, w.y), __fmul2_rn(a, make_float2(w.x, w.x)));
-}
-PTY_DEV float2 cmulc_tw(float2 w, float2 a) {     // conj(w) * a
-    return __ffma2_rn(make_float2(a.y, a.x), make_float2(w.y, -w.y), __fmul2_rn(a, make_float2(w.x, w.x)));
-}
-#else
+// variable twiddles of the cross-thread radix-4 stage (scalar form: the packed one measured +-0)
 PTY_DEV float2 cmul_tw(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
 PTY_DEV float2 cmulc_tw(float2 w, float2 a) { return make_float2(w.x * a.x + w.y * a.y, w.x * a.y - w.y * a.x); }
-#endif
 
 // a * exp(DIR * i * pi/2): forward multiplies by -i, inverse by +i
 template <int DIR> PTY_DEV float2 mul_qi(float2 a) {
@@ -90,14 +44,9 @@ template <int DIR> PTY_DEV float2 mul_qi(float2 a) {
 }
 // a * (c + i*DIR*s) with c, s the cos/sin of a positive angle
 template <int DIR> PTY_DEV float2 mul_cs(float2 a, float c, float s) {
-#if PTY_PK_CS
     const float2 t = __fmul2_rn(a, make_float2(c, c));
     return DIR < 0 ? __ffma2_rn(make_float2(a.y, a.x), make_float2(s, -s), t)
                    : __ffma2_rn(make_float2(a.y, a.x), make_float2(-s, s), t);
-#else
-    return DIR < 0 ? make_float2(a.x * c + a.y * s, a.y * c - a.x * s)
-                   : make_float2(a.x * c - a.y * s, a.y * c + a.x * s);
-#endif
 }
 
 // ----------------------------------------------------------------------------- radix-4 / 8 / 16
@@ -158,7 +107,6 @@ template <int DIR> struct RegFFT<16, DIR> {
 // ----------------------------------------------------------------------------- shapes
 template <int N_> struct Shape;
 template <> struct Shape<64>  { static constexpr int N = 64,  R1 = 8,  R2 = 8,  CL = 1, NL = 64,  NT = 256; };
-template <> struct Shape<128> { static constexpr int N = 128, R1 = 16, R2 = 8,  CL = 1, NL = 128, NT = 512; };
 template <> struct Shape<256> { static constexpr int N = 256, R1 = 16, R2 = 16, CL = 4, NL = 64,  NT = 512; };
 
 template <class SH> struct ShapeInfo {
@@ -219,11 +167,7 @@ template <class SH> PTY_DEV void sync_all_war() {
 template <class SH, int DIR, class In>
 PTY_DEV void stage_a(const Cta<SH>& c, In& in) {
     using I = ShapeInfo<SH>;
-#if PTY_STAGE_A_UNROLL
 #pragma unroll
-#else
-#pragma unroll 1
-#endif
     for (int it = 0; it < I::TA; ++it) {
         const int t = it * I::NT + c.tid;
         const int line = t % I::NL, n2 = t / I::NL;
@@ -276,10 +220,8 @@ PTY_DEV void stage_b_exchange(const Cta<SH>& c, float2 (&v)[ShapeInfo<SH>::TB][S
         unsigned rbase;
         asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbase)
                      : "r"((unsigned)__cvta_generic_to_shared(c.S + (size_t)(RANK * I::NL) * I::PITCH)), "r"(d));
-#if PTY_DSMEM_ASYNC
         unsigned rbar;
         asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbar) : "r"((unsigned)__cvta_generic_to_shared(c.rx)), "r"(d));
-#endif
         float2 tv[(I::NL * I::NL) / I::NT];
 #pragma unroll
         for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
@@ -290,14 +232,10 @@ PTY_DEV void stage_b_exchange(const Cta<SH>& c, float2 (&v)[ShapeInfo<SH>::TB][S
         for (int j = 0; j < (I::NL * I::NL) / I::NT; ++j) {
             const int idx = j * I::NT + c.tid;
             const unsigned a = rbase + (unsigned)(((idx / I::NL) * I::PITCH + idx % I::NL) * sizeof(float2));
-#if PTY_DSMEM_ASYNC
             // asynchronous remote store: its 8 bytes are counted on the RECEIVER's mbarrier, so the exchange needs neither
             // a release fence (which would also drain this thread's saved-wave stores to HBM) nor a closing cluster barrier
             asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
                          ::"r"(a), "f"(tv[j].x), "f"(tv[j].y), "r"(rbar) : "memory");
-#else
-            asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(tv[j].x), "f"(tv[j].y) : "memory");
-#endif
         }
     }
 }
@@ -345,26 +283,22 @@ PTY_DEV void stage_b(const Cta<SH>& c) {
         // The NL x NL tile that goes to CTA d is first assembled in local shared memory (scattered 8-byte stores,
         // cheap locally) and then copied to the owner with lane-contiguous stores: a warp writes 256 contiguous
         // bytes of remote shared memory instead of 32 separate 8-byte words (the scattered form ran at 10 % issue
-        // utilisation, stalled on lg_throttle -- profiles/r01_v4_fwd256).  Two tiles alternate, one CTA barrier
+        // utilisation, stalled on lg_throttle -- round 1).  Two tiles alternate, one CTA barrier
         // per destination; destinations start at the own rank so that the four CTAs do not target one peer.
         // The rank is a template parameter of the exchange (a CTA-uniform switch), so the destination of every register
         // is known at compile time: no predicated-off stores, and the tile for the own CTA is written in place.
-#if PTY_DSMEM_ASYNC
         // this CTA expects the tiles of its CL - 1 peers (one arrival: this post; the bytes: their st.async)
         if (c.tid == 0) mbar_expect_tx(c.rx, (unsigned)((SH::CL - 1) * I::NL * I::NL * sizeof(float2)));
-#endif
         switch (c.rank) {
             case 0: stage_b_exchange<SH, 0>(c, v); break;
             case 1: stage_b_exchange<SH, 1 % SH::CL>(c, v); break;
             case 2: stage_b_exchange<SH, 2 % SH::CL>(c, v); break;
             default: stage_b_exchange<SH, 3 % SH::CL>(c, v); break;
         }
-#if PTY_DSMEM_ASYNC
         mbar_wait(c.rx, c.rx_phase);      // every peer's tile has landed in this CTA's wave
         c.rx_phase ^= 1u;
         pty_cta_sync();                   // ... and this CTA's own tile (written in place by its threads)
         return;
-#endif
     }
     sync_all<SH>();
 }

@@ -56,30 +56,10 @@ struct Cta128 {
     PTY_DEV int kx(int r) const { return 8 * (tid >> 7) + (r & 7) + 32 * (r >> 3); }
 };
 
-// cos / sin of 2 pi j / 32
-PTY_DEV constexpr float c32(int j) {
-    constexpr float t[9] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
-                            0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
-                            0.19509032201612826785f, 0.0f};
-    j &= 31;
-    return j <= 8 ? t[j] : j <= 16 ? -t[16 - j] : j <= 24 ? -t[j - 16] : t[32 - j];
-}
-PTY_DEV constexpr float s32(int j) { return c32(j - 8); }
-
-template <int J, int DIR> PTY_DEV float2 mul_w32(float2 a) {
-    constexpr float c = c32(J), s = s32(J);
-    if constexpr (J % 32 == 0) return a;
-    else if constexpr (J % 32 == 8) return mul_qi<DIR>(a);
-    else return mul_cs<DIR>(a, c, s);
-}
-
-// ---- FMA-form twiddles.  w u = gamma (alpha u + beta (i u)) with |alpha|, |beta| <= 1 and one of them 1: the inner
+// ---- FMA-form twiddles (cos / sin of 2 pi j / 32 as compile-time constants).  w u = gamma (alpha u + beta (i u)) with |alpha|, |beta| <= 1 and one of them 1: the inner
 // bracket u' is ONE packed FMA, and the real scale gamma is carried as "pending" into the add/sub pair that consumes
 // the value (y +- gamma u' = two packed FMAs instead of two packed adds): 3 packed instructions per twiddled
 // butterfly input instead of 4, and no extra rounding step.  All constants are compile-time.
-#ifndef PTY_FMA_FORM
-#define PTY_FMA_FORM 1
-#endif
 PTY_DEV constexpr double cd32(int j) {
     constexpr double t[9] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
                              0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
@@ -181,7 +161,6 @@ struct NoBg { template <int K> PTY_DEV void tick() {} };
 template <int DIR, int TB, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg) {
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) bfly4<DIR>(v[n2], v[8 + n2], v[16 + n2], v[24 + n2]);   // -> v[8 k1 + n2]
-#if PTY_FMA_FORM
     bg.template tick<TB>();
     {
         float2 o[32];
@@ -199,30 +178,7 @@ template <int DIR, int TB, class BG> PTY_DEV void fft32(float2 (&v)[32], BG& bg)
 #undef PTY_F8
 #pragma unroll
         for (int k = 0; k < 32; ++k) v[k] = o[k];
-        return;
     }
-#endif
-#define PTY_TW(K1, N2) v[8 * K1 + N2] = mul_w32<K1 * N2, DIR>(v[8 * K1 + N2]);
-    PTY_TW(1, 1) PTY_TW(1, 2) PTY_TW(1, 3) PTY_TW(1, 4) PTY_TW(1, 5) PTY_TW(1, 6) PTY_TW(1, 7)
-    PTY_TW(2, 1) PTY_TW(2, 2) PTY_TW(2, 3) PTY_TW(2, 4) PTY_TW(2, 5) PTY_TW(2, 6) PTY_TW(2, 7)
-    PTY_TW(3, 1) PTY_TW(3, 2) PTY_TW(3, 3) PTY_TW(3, 4) PTY_TW(3, 5) PTY_TW(3, 6) PTY_TW(3, 7)
-#undef PTY_TW
-    bg.template tick<TB>();
-    float2 o[32];
-#pragma unroll
-    for (int k1 = 0; k1 < 4; ++k1) {
-        float2 w[8];
-#pragma unroll
-        for (int n2 = 0; n2 < 8; ++n2) w[n2] = v[8 * k1 + n2];
-        RegFFT<8, DIR>::run(w);
-#pragma unroll
-        for (int k2 = 0; k2 < 8; ++k2) o[k1 + 4 * k2] = w[k2];
-        if (k1 == 0) bg.template tick<TB + 1>();
-        if (k1 == 1) bg.template tick<TB + 2>();
-        if (k1 == 2) bg.template tick<TB + 3>();
-    }
-#pragma unroll
-    for (int k = 0; k < 32; ++k) v[k] = o[k];
 }
 
 // twiddle table (forward sign), filled once per CTA: twg[g][i][q] = W128^(q (8 g + i))

@@ -22,14 +22,8 @@
 #include "pty_fft128.cuh"
 #include "pty_kernels.cuh"
 
-#ifndef PTY_G2_EARLY
-#define PTY_G2_EARLY 0  // request the first D saved-wave chunks before the park phase's inverse transforms
-#endif
 #ifndef PTY_G2_PAIR_NS
 #define PTY_G2_PAIR_NS 4   // chunk slots of the pair-sum ring (8 KB each); measured on c4: 2 -> 6.27 ms, 4 -> 6.13 ms, 8 -> 7.30 ms (L1 shrinks)
-#endif
-#ifndef PTY_G2_FLIP
-#define PTY_G2_FLIP 1
 #endif
 #ifndef PTY_G2_D
 #define PTY_G2_D 3      // chunks of saved-wave / object rows in flight in the adjoint's streaming step
@@ -37,60 +31,28 @@
 
 namespace pty {
 
-// timing ablations (never defined in the product build): drop one memory stream of the adjoint's streaming step
+// the memory streams of the adjoint's streaming step, one helper each
 PTY_DEV void g2_red_obj(float2* p, float2 v) {
-#ifdef PTY_ABL_RED
-    if (v.x == 1.2345e-30f)
-#endif
     red_add2(p, v);
 }
 PTY_DEV float4 g2_ld_psi(const float4* p) {
-#ifdef PTY_ABL_PSI
-    return make_float4(1.f, 2.f, 3.f, 0.5f);
-#else
     return ld_stream4_pinned(p);
-#endif
 }
 PTY_DEV float2 g2_ld_obj(const float2* p) {
-#ifdef PTY_ABL_OBJ
-    return make_float2(0.9f, 0.1f);
-#else
     return ldg2_pinned(p);
-#endif
 }
 
 PTY_DEV void g2_st_psi(float4* p, float2 a, float2 b) {
-#ifdef PTY_ABL_PSI
-    if (a.x == 1.2345e-30f)
-#endif
     st_stream4(p, a, b);
 }
-
-// timeline instrumentation (never defined in the product build): lane 0 of every warp of CTA 0 logs (event id, SM clock)
-#ifdef PTY_TRACE
-__device__ long long g_trace[16 * 1024];
-__device__ int g_trace_n[16];
-PTY_DEV void g2_trace(int ev) {
-    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {
-        const int w = threadIdx.x >> 5;
-        const int n = g_trace_n[w];
-        if (n < 1024) { g_trace[w * 1024 + n] = ((long long)ev << 48) | (clock64() & 0xffffffffffffLL); g_trace_n[w] = n + 1; }
-    }
-}
-#else
-PTY_DEV void g2_trace(int) {}
-#endif
 
 struct G2Smem {
     static constexpr size_t xch_bytes = F128::xch_bytes;
     // twg[128] | per group: Ey, Ex, My, Mx [128 each] float2, red[64] float | TMEM base
     static constexpr size_t group_bytes = 4 * 128 * sizeof(float2) + 64 * sizeof(float);
-#ifndef PTY_ABL_SMEM_PAD
-#define PTY_ABL_SMEM_PAD 0      // timing ablation: extra dynamic shared memory (shrinks L1)
-#endif
     // twf[32][12]: FMA-form constants of the forward radix-4 stage (g2_radix4<-1>)
     static constexpr size_t twf_bytes = 32 * 12 * sizeof(float);
-    static constexpr size_t bytes = xch_bytes + 128 * sizeof(float2) + 2 * group_bytes + 16 + twf_bytes + PTY_ABL_SMEM_PAD;
+    static constexpr size_t bytes = xch_bytes + 128 * sizeof(float2) + 2 * group_bytes + 16 + twf_bytes;
 };
 
 struct G2 {
@@ -109,13 +71,8 @@ struct G2 {
         tmem_fence_after_sync();
     }
     PTY_DEV void grp_sync() const { asm volatile("bar.sync %0, 256;" ::"r"(9 + G) : "memory"); }
-#if defined(PTY_ABL_ONEGROUP) || defined(PTY_ABL_NOX)   // timing ablations: no hand-over of the transpose buffer
-    PTY_DEV void acquireX() const {}
-    PTY_DEV void releaseX() const {}
-#else
     PTY_DEV void acquireX() const { asm volatile("bar.sync %0, 512;" ::"r"(11 + G) : "memory"); }
     PTY_DEV void releaseX() const { asm volatile("bar.arrive %0, 512;" ::"r"(11 + (G ^ 1)) : "memory"); }
-#endif
 };
 
 PTY_DEV G2 make_g2(unsigned char* smem) {
@@ -261,7 +218,6 @@ PTY_DEV void g2_item_rows(const KArgs& A, int item, int o, int& row0, int& rx) {
 // DIR < 0: v[8 q + i] -> twiddle W128^(q (8 o + i)) -> radix-4 over q -> v[8 k2 + i]   (forward)
 // DIR > 0: v[8 k2 + i] -> inverse radix-4 over k2 -> conj twiddle -> v[8 q + i]         (inverse)
 template <int DIR> PTY_DEV void g2_radix4(const G2& c, int o, float2 (&v)[32]) {
-#if PTY_FMA_FORM
     if constexpr (DIR < 0) {
         // FMA form (pty_fft128.cuh): the three twiddled inputs cost one packed FMA each, their real scales ride on the
         // butterfly's add/sub pairs: 11 packed FMAs per butterfly instead of 12 scalar + 8 packed instructions
@@ -272,7 +228,6 @@ template <int DIR> PTY_DEV void g2_radix4(const G2& c, int o, float2 (&v)[32]) {
         }
         return;
     }
-#endif
     const float4* tw = reinterpret_cast<const float4*>(c.twg + 32 * o);
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
@@ -322,10 +277,8 @@ PTY_DEV void g2_st_slots(const G2& c, int o, float2 (&v)[32]) {
 PTY_DEV void g2_inverse_head(const G2& c, float2 (&v)[32], bool first) {
     constexpr int P = F128::P;
     NoBg bg;
-    g2_trace(1);
     c.pair_sync();
     if (!first) c.acquireX();
-    g2_trace(2);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -335,9 +288,7 @@ PTY_DEV void g2_inverse_head(const G2& c, float2 (&v)[32], bool first) {
 #pragma unroll
         for (int n = 0; n < 32; ++n) s[4 * n] = v[n];
     }
-    g2_trace(3);
     c.grp_sync();
-    g2_trace(4);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -349,14 +300,12 @@ PTY_DEV void g2_inverse_head(const G2& c, float2 (&v)[32], bool first) {
             v[16 + i] = s[(i + 64) * P];
             v[24 + i] = s[(i + 96) * P];
         }
-        if (h == 1) { c.releaseX(); g2_trace(5); }
+        if (h == 1) c.releaseX();
         g2_radix4<+1>(c, o, v);
         g2_st_slots(c, o, v);
     }
     tmem_wait_st();
-    g2_trace(6);
     c.pair_sync();
-    g2_trace(7);
 }
 
 // Forward transform after the per-role fft32<-1> + g2_st_own of the caller: role blocks -> y radix-4 -> X ->
@@ -365,10 +314,8 @@ PTY_DEV void g2_forward_tail(const G2& c, float2 (&v)[32]) {
     constexpr int P = F128::P;
     NoBg bg;
     tmem_wait_st();
-    g2_trace(8);
     c.pair_sync();
     c.acquireX();
-    g2_trace(9);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -378,9 +325,7 @@ PTY_DEV void g2_forward_tail(const G2& c, float2 (&v)[32]) {
 #pragma unroll
         for (int r = 0; r < 32; ++r) s[((r & 7) + 32 * (r >> 3)) * P] = v[r];
     }
-    g2_trace(10);
     c.grp_sync();
-    g2_trace(11);
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int o = 2 * c.gg + h;
@@ -392,14 +337,12 @@ PTY_DEV void g2_forward_tail(const G2& c, float2 (&v)[32]) {
             v[16 + n2] = s[4 * (16 + n2)];
             v[24 + n2] = s[4 * (24 + n2)];
         }
-        if (h == 1) { c.releaseX(); g2_trace(12); }
+        if (h == 1) c.releaseX();
         fft32<-1, 0>(v, bg);
         g2_st_own(c, o, v);
     }
     tmem_wait_st();
-    g2_trace(13);
     c.pair_sync();
-    g2_trace(14);
 }
 
 PTY_DEV void g2_accumulate(const G2& c, int slot, float v) {
@@ -424,7 +367,6 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
     int ry, rx;
     setup_factors<128, 256>(c.t, c.Ey, c.Ex, c.My, c.Mx, c.red, A, b, ry, rx);
     c.grp_sync();
-    g2_trace(20);
     const size_t NN = (size_t)N * N;
     const size_t bm = (size_t)slot;
     float2 v[32];
@@ -442,7 +384,6 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
         }
         tmem_wait_st();
     }
-    g2_trace(21);
     bool first = (c.G == 0);
     for (int s = 0; s < A.Nz; ++s) {
         g2_inverse_head(c, v, first);
@@ -450,7 +391,7 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
         // a3 + a4 (R): psi_{s-1} = fft32^-1, keep it, phi_s = O_b[s] psi_{s-1}, first stage of the forward y transform
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
-            const int o = 2 * c.gg + (TMA || !PTY_G2_FLIP ? h : (h ^ c.G));   // group 1 takes its roles in the opposite order: its object rows are then the ones group 0 read last (L1 hits)
+            const int o = 2 * c.gg + (TMA ? h : (h ^ c.G));   // group 1 takes its roles in the opposite order: its object rows are then the ones group 0 read last (L1 hits)
             const float2* obj = A.object + obj_off + ((size_t)s * A.H + ry + o) * A.W + rx + c.c;
             const size_t ostride = (size_t)4 * A.W;
             float2 oa[8], ob[8];
@@ -550,7 +491,6 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
             g2_st_slots(c, o, v);
         }
         tmem_wait_st();
-        g2_trace(23);
     }
     // a5 (K): Psi = F[phi_Nz] / N, I += |Psi|^2.  I is kept in thread order as pairs, [r / 2][128 o + ky][r & 1]
     // (layout K: register r of role o holds k_x = 8 o + (r & 7) + 32 (r >> 3)): one 8-byte vector RED per two
@@ -570,7 +510,6 @@ PTY_DEV void fwd_body_g2(const KArgs& A, const G2& c, G2Ring& ring, int item, in
             red_add2(Ib + (r >> 1) * NT + 128 * o + c.c, make_float2(p0.x * p0.x + p0.y * p0.y, p1.x * p1.x + p1.y * p1.y));
         }
     }
-    g2_trace(24);
     if (c.G == 0) c.acquireX();      // consume group 1's last release
 }
 
@@ -601,7 +540,6 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
         tmem_wait_st();
     }
     float acc_ky = 0.f, acc_kx = 0.f, acc_k2 = 0.f;
-    g2_trace(31);
     bool first = (c.G == 0);
     for (int s = A.Nz - 1; s >= 0; --s) {
         g2_inverse_head(c, v, first);
@@ -609,15 +547,14 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
         // a9, a10 (R): g = fft32^-1; g_object patch += conj(psi_{s-1}) g; g <- conj(O_b[s]) g; forward y first stage.
         // Park-then-stream: both roles' g goes back to its TMEM block first, which frees the 64 wave registers;
         // the pointwise step then streams over the 16 chunks of 4 rows (two roles x 8) with the saved wave (HBM
-        // stream) and the object rows D chunks ahead in registers and g one chunk ahead from TMEM.  The first D
-        // chunks of the saved wave are requested BEFORE the two inverse fft32 of the park phase (PTY_G2_EARLY):
-        // that arithmetic covers the HBM latency of the stream's start.
+        // stream) and the object rows D chunks ahead in registers and g one chunk ahead from TMEM.  (Requesting the first
+        // D saved-wave chunks before the park phase's inverse fft32 measured -4 %: round 2.)
         constexpr int D = PTY_G2_D;
         const float4* psi0 = reinterpret_cast<const float4*>(A.ws_psi + (bm * A.Nz + s) * NN) + 256 * c.gg + c.c;
         float4 pb[D][2];
         // group 1 streams its two roles in the opposite order: the object rows it reads are then the ones group 0 (same
         // position, the neighbouring mode) has read last, and they are still in L1
-        const int fl = (PTY_G2_FLIP && !PAIR) ? c.G : 0;     // pair sum: both groups must walk the rows in one order
+        const int fl = !PAIR ? c.G : 0;     // pair sum: both groups must walk the rows in one order
         const int pr0 = fl ? 128 : 0, pr1 = 128 - pr0;                      // saved-wave offset of the first / second role
         const size_t or0 = fl ? (size_t)A.W : 0, or1 = (size_t)A.W - or0;   // object-row offset
         const unsigned tr0 = fl ? 64u : 0u, tr1 = 64u - tr0;                // TMEM role block
@@ -627,12 +564,6 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
             pb[(J) % D][0] = g2_ld_psi(pp_);                                                              \
             pb[(J) % D][1] = g2_ld_psi(pp_ + NT);                                                         \
         }
-#if PTY_G2_EARLY
-        PTY_G2_ISSUE_PSI(0) PTY_G2_ISSUE_PSI(1) PTY_G2_ISSUE_PSI(2)
-        if (D > 3) PTY_G2_ISSUE_PSI(3)
-        if (D > 4) PTY_G2_ISSUE_PSI(4)
-        if (D > 5) PTY_G2_ISSUE_PSI(5)
-#endif
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
             const int o = 2 * c.gg + h;
@@ -641,7 +572,6 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
             g2_st_own(c, o, v);
         }
         tmem_wait_st();
-        g2_trace(32);
         {
             const size_t ostride = (size_t)4 * A.W;
             const float2* obj0 = A.object + obj_off + ((size_t)s * A.H + ry + 2 * c.gg) * A.W + rx + c.c;
@@ -654,11 +584,7 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
                 const float2* oo_ = obj0 + ((J) >> 3 ? or1 : or0) + (size_t)(4 * ((J) & 7)) * ostride;    \
                 _Pragma("unroll") for (int i = 0; i < 4; ++i) ob[(J) % D][i] = g2_ld_obj(oo_ + (size_t)i * ostride); \
             }
-#if PTY_G2_EARLY
-#define PTY_G2_ISSUE(J) { PTY_G2_ISSUE_OBJ(J) }
-#else
 #define PTY_G2_ISSUE(J) { PTY_G2_ISSUE_PSI(J) PTY_G2_ISSUE_OBJ(J) }   // one statement: used under `if (D > n)`
-#endif
 #define PTY_G2_STEP(J)                                                                                    \
             {                                                                                             \
                 tmem_wait_ld();                                                                           \
@@ -708,7 +634,6 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
 #undef PTY_G2_ISSUE_PSI
         }
         tmem_wait_st();
-        g2_trace(33);
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
             const int o = 2 * c.gg + h;
@@ -716,7 +641,6 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
             fft32<-1, 0>(v, bg);
             g2_st_own(c, o, v);
         }
-        g2_trace(34);
         g2_forward_tail(c, v);
         if (s == 0) break;
         // a9, a13 (K): D-sums against the kept spectrum, conj(M), inverse x radix-4, in-place slots
@@ -745,7 +669,6 @@ template <bool HAT, bool PAIR> PTY_DEV void bwd_body_g2(const KArgs& A, const G2
             g2_st_slots(c, o, v);
         }
         tmem_wait_st();
-        g2_trace(35);
     }
     // a11, a12 (K): g^_0 = F[g_psi0]; probe-gradient accumulation and the position gradient
     float accy = 0.f, accx = 0.f;

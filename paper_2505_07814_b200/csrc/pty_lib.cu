@@ -112,9 +112,6 @@ __global__ void __launch_bounds__(F128::NT, 1) pty_fwd128g2_kernel(const KArgs A
     }
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         const int item = it + c.G;
-#ifdef PTY_ABL_ONEGROUP
-        if (c.G == 1) break;
-#endif
         const int itn = it + 2 * (int)gridDim.x;
         fwd_body_g2<HAT, TMA>(A, c, ring, min(item, n - 1), item, item < n ? 1.f : 0.f,   // item == n: the ghost (slot n)
                               itn < n ? min(itn + c.G, n - 1) : -1);
@@ -133,9 +130,6 @@ template <bool HAT, bool PAIR> __global__ void __launch_bounds__(F128::NT, 1) pt
     const int n = A.B * A.MT;
     for (int it = 2 * blockIdx.x; it < n; it += 2 * gridDim.x) {
         int item = it + c.G;
-#ifdef PTY_ABL_ONEGROUP
-        if (c.G == 1) break;
-#endif
         bwd_body_g2<HAT, PAIR>(A, c, pr, min(item, n - 1), item, item < n ? 1.f : 0.f);
         c.grp_sync();
     }
@@ -1306,15 +1300,4 @@ int64_t pty_launch_count(const pty_plan* plan) { return plan ? plan->launches : 
 
 const char* pty_last_error(const pty_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
 
-#ifdef PTY_TRACE
-// timeline instrumentation (debug builds only): copies the trace of CTA 0 out and resets it
-int pty_trace_read(long long* host_events, int* host_counts) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(host_events, pty::g_trace, sizeof(long long) * 16 * 1024);
-    cudaMemcpyFromSymbol(host_counts, pty::g_trace_n, sizeof(int) * 16);
-    int zero[16] = {0};
-    cudaMemcpyToSymbol(pty::g_trace_n, zero, sizeof(zero));
-    return 0;
-}
-#endif
 }  // extern "C"
