@@ -534,3 +534,83 @@ def test_step_ap_and_constraints_replay_as_one_cuda_graph(pty):
         assert rel_l2(a - z, b - z) <= 2e-2, nm           # the few pixels with |g| ~ rounding may step the other way
         assert rel_l2(a, b) <= 1e-4, nm
     assert plan.status()[0] == 0
+
+
+# ----------------------------------------------------------------------------- shapes the round-2 verdict found untested
+def _tilt_case(name):
+    if name == "c5_global_tilt_n256":          # 256^2 cluster path, one tilt for the minibatch (config 5's own mode)
+        return small_case(5, 2, Nz=2, M=2)
+    if name == "c3_tilt_per_position":         # tilt_mode 2 at full c3 depth
+        idx = synth.minibatch(synth.get_config(3), 1, 512)[:4]
+        return make_case(3, "A", idx, tilt_mode=2)
+    raise KeyError(name)
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("name", ["c5_global_tilt_n256", "c3_tilt_per_position"])
+def test_amplitude_phase_object_with_tilt(pty, name):
+    """pty_*_ap with a tilted propagator (Eq. 4; amplitude / phase object PAPER.md:114): the tilt and
+    dz gradients pass through the composed object unchanged.  tilt_mode 1 at N = 256 and tilt_mode 2 at N = 128, the
+    full Eq. 9 with sparsity; every gradient against the oracle."""
+    case = _tilt_case(name)
+    cfg, tm = case["cfg"], case["tilt_mode"]
+    B = len(case["positions"])
+    amp, phase = _amp_phase_of(case["object"])
+    w = ol.LossWeights(1.0, 0.4, 0.6, 0.1)
+    ref = ol.total_loss_and_gradients(None, case["probe"], case["positions"], case["tilt"], case["meas"], geom_of(cfg), w,
+                                      amp=amp, phase=phase)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, tilt_mode=tm, flags=pty.PTY_FLAG_AMP_PHASE)
+    plan.set_loss(1, w.gaussian, w.poisson, w.pacbed, w.sparse, w.eps)
+    tA, tp, probe, pos, meas = dev(amp), dev(phase), dev(case["probe"]), dev(case["positions"]), dev(case["meas"])
+    tilt = dev(np.asarray(case["tilt"], np.float32))
+    loss = plan.forward_loss_ap(tA, tp, probe, pos, tilt, meas)
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
+    gA, gp = torch.full_like(tA, 7.0), torch.full_like(tp, 7.0)
+    g_probe, g_pos = torch.zeros_like(probe), torch.zeros(B, 2, device="cuda")
+    g_tilt = torch.zeros((B, 2) if tm == 2 else (2,), device="cuda")
+    g_dz = torch.zeros(1, device="cuda")
+    plan.backward_ap(tA, tp, probe, pos, tilt, meas, gA, gp, g_probe, g_pos, g_tilt, g_dz)
+    assert plan.status()[0] == 0
+    errs = {"g_amp": rel_l2(gA.cpu().numpy(), ref["g_amp"]), "g_phase": rel_l2(gp.cpu().numpy(), ref["g_phase"]),
+            "g_probe": rel_l2(g_probe.cpu().numpy(), ref["g_probe"]), "g_positions": rel_l2(g_pos.cpu().numpy(), ref["g_positions"]),
+            "g_tilt": rel_l2(g_tilt.cpu().numpy(), ref["g_tilt"] if tm == 2 else ref["g_tilt"].sum(0)),
+            "g_dz": abs(g_dz.item() - ref["g_dz"]) / abs(ref["g_dz"])}
+    print(name, " ".join(f"{k} {v:.2e}" for k, v in errs.items()))
+    assert all(v <= GRAD_RTOL for v in errs.values()), errs
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("name", ["c5_n256_global_tilt", "c3_spectra_flag"])
+def test_mixed_object_states_with_spectra(pty, name):
+    """n_obj = 2 (Eq. 2) on the kernels that keep the propagated spectra: the N = 256 cluster path with
+    config 5's global tilt (g_tilt, g_dz), and N = 128 with PTY_FLAG_SPECTRA (g_dz without tilt).  Eq. 9 loss; every
+    gradient, g_object per state, against the oracle."""
+    if name == "c5_n256_global_tilt":
+        case, flags = small_case(5, 2, Nz=2, M=2), 0
+    else:
+        case, flags = small_case(3, 4, Nz=3, M=3), pty.PTY_FLAG_SPECTRA
+    cfg, tm = case["cfg"], case["tilt_mode"]
+    B = len(case["positions"])
+    rng = np.random.default_rng(29)
+    second = case["object"] * np.exp(1j * 0.1 * rng.standard_normal(case["object"].shape)).astype(np.complex64)
+    obj2 = np.ascontiguousarray(np.stack([case["object"], second * 0.6]).astype(np.complex64))
+    w = ol.LossWeights(1.0, 0.4, 0.6, 0.0)
+    ref = ol.total_loss_and_gradients(obj2, case["probe"], case["positions"], case["tilt"], case["meas"], geom_of(cfg), w)
+    plan = pty.Plan(cfg.Nz, cfg.H, cfg.W, cfg.M, cfg.N, B, cfg.dz, cfg.lam, cfg.dx, tilt_mode=tm, flags=flags, n_obj=2)
+    plan.set_loss(1, w.gaussian, w.poisson, w.pacbed, 0.0, w.eps)
+    o, probe, pos, meas = dev(obj2), dev(case["probe"]), dev(case["positions"]), dev(case["meas"])
+    tilt = dev(np.asarray(case["tilt"], np.float32)) if tm else None
+    loss = plan.forward_loss(o, probe, pos, tilt, meas)
+    g_obj, g_probe, g_pos = torch.zeros_like(o), torch.zeros_like(probe), torch.zeros(B, 2, device="cuda")
+    g_tilt = torch.zeros(2, device="cuda") if tm else None
+    g_dz = torch.zeros(1, device="cuda")
+    plan.backward(o, probe, pos, tilt, meas, g_obj, g_probe, g_pos, g_tilt, g_dz, flags=pty.PTY_BWD_REUSE_FORWARD)
+    assert plan.status()[0] == 0
+    assert abs(loss.item() - ref["loss"]) <= LOSS_RTOL * abs(ref["loss"])
+    errs = {f"g_object[{n}]": rel_l2(g_obj[n].cpu().numpy(), ref["g_object"][n]) for n in range(2)}
+    errs.update({"g_probe": rel_l2(g_probe.cpu().numpy(), ref["g_probe"]), "g_positions": rel_l2(g_pos.cpu().numpy(), ref["g_positions"]),
+                 "g_dz": abs(g_dz.item() - ref["g_dz"]) / abs(ref["g_dz"])})
+    if tm:
+        errs["g_tilt"] = rel_l2(g_tilt.cpu().numpy(), ref["g_tilt"].sum(0))
+    print(name, " ".join(f"{k} {v:.2e}" for k, v in errs.items()))
+    assert all(v <= GRAD_RTOL for v in errs.values()), errs
