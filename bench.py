@@ -257,6 +257,9 @@ def main():
                     help="replay each step (forward + gradient of one minibatch) as one CUDA graph; auto = on for the "
                          "launch-bound small configurations 1 and 2 on one GPU")
     ap.add_argument("--e2e-plans", type=int, default=3, help="plans / streams of the pipelined end-to-end measurement")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend for --gpus > 1; gloo (with ranks wrapping around the visible GPUs) "
+                         "only exists to exercise the multi-rank code path on a box with fewer GPUs than ranks")
     ap.add_argument("--plan-flags", type=int, default=0,
                     help="extra pty_dims.flags for the timed plan (16 = PTY_FLAG_TMA_OBJECT, 32 = PTY_FLAG_PAIR_SUM): "
                          "opt-in kernel variants, reported in config.plan_flags")
@@ -281,9 +284,14 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference for the oracle)")
+    if args.dist_backend == "gloo":
+        local %= torch.cuda.device_count()
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
     dev = torch.device("cuda", local)
 
     # ---- synthetic dataset: truth -> measurements (library forward + Poisson), evaluation point A
@@ -311,18 +319,27 @@ def main():
     del obj_t, probe_t, inten, zeros
 
     g_obj, g_probe = torch.zeros_like(obj), torch.zeros_like(probe)
-    g_pos = torch.zeros(B, 2, device=dev)
+    # N ranks: one global minibatch of N * B positions per step, rank r owning rows [r B, (r + 1) B) (weak scaling), combined
+    # by the library's own data-parallel host logic (parallel.sharded_gradient: one sum all-reduce of the partial
+    # object / probe / tilt gradients, the loss and the position-gradient rows)
+    g_pos_all = torch.zeros(world * B, 2, device=dev)
+    g_pos = g_pos_all[rank * B:(rank + 1) * B]
     g_tilt = torch.zeros(2, device=dev) if cfg.tilt_mode else None
     loss = torch.zeros(1, dtype=torch.float64, device=dev)
 
-    def step(i):
+    def step_local(i):
         j = i % n_used
         plan.forward_loss(obj, probe, pos_batches[j], tilt, meas_batches[j], loss)
         plan.backward(obj, probe, pos_batches[j], tilt, meas_batches[j], g_obj, g_probe, g_pos, g_tilt,
                       flags=binding.PTY_BWD_REUSE_FORWARD)
-        if world > 1:
-            dist.all_reduce(torch.view_as_real(g_obj))
-            dist.all_reduce(torch.view_as_real(g_probe))
+
+    def step(i):
+        if world == 1:
+            step_local(i)
+        else:
+            from paper_2505_07814_b200 import parallel
+            span = parallel.sharded_gradient(lambda lo, hi: step_local(i), world * B, g_obj, g_probe, g_pos_all, g_tilt, loss)
+            assert span == (rank * B, (rank + 1) * B)
 
     def barrier():
         torch.cuda.synchronize()
@@ -392,7 +409,7 @@ def main():
         h_go, h_gp = torch.zeros_like(h_obj).pin_memory(), torch.zeros_like(h_probe).pin_memory()
         h_gq = torch.zeros(B, 2).pin_memory()
         h_gt = torch.zeros(2).pin_memory() if tilt is not None else None
-        k_e2e = max(2, min(args.steps, 5))
+        k_e2e = max(2, min(args.steps, 12))
         run = lambda i: plan.grad_host(h_obj, h_probe, h_pos[i % len(h_pos)], h_tilt, h_meas[i % len(h_meas)], h_loss,
                                        h_go, h_gp, h_gq, h_gt)
         run(0)
@@ -421,7 +438,7 @@ def main():
                 plans[k].grad_host(h_obj, h_probe, h_pos[i % len(h_pos)], h_tilt, h_meas[i % len(h_meas)], *outs[k],
                                    wait=False)
 
-        k_pipe = NP * max(2, min(args.steps, 8) // 2)
+        k_pipe = NP * max(2, min(args.steps, 24) // 2)
         for i in range(NP):
             enqueue(i)
             plans[i].grad_host_wait()
@@ -499,6 +516,10 @@ def main():
         if os.path.exists(tp):
             try:
                 roofline["traffic"] = json.load(open(tp)).get(f"c{cfg.c}_B{B}_{dom}")
+                if roofline["traffic"] is not None:
+                    roofline["traffic_source"] = ("stored figure, not measured by this run: dram__bytes_read.sum + "
+                                                  "dram__bytes_write.sum of one `ncu --set full` capture of this kernel "
+                                                  "(profiles/traffic.json)")
             except Exception:
                 pass
 
