@@ -119,6 +119,16 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def oracle_per_core(oracle, ev, pos, tilt_e, meas, geom, cores):
+    """The oracle on ONE core (workers = 1, a few positions): patterns/s per core and what `cores` perfectly scaling
+    workers would give, so that the multi-process figure beside it can be judged."""
+    m = max(1, min(3, len(pos)))
+    t0 = time.perf_counter()
+    oracle.grad_batch(ev["object"], ev["probe"], pos[:m], tilt_e, meas[:m], geom, workers=1)
+    per_core = m / (time.perf_counter() - t0)
+    return {"per_core": per_core, "positions_timed": m, "ideal_all_cores": per_core * cores}
+
+
 # ------------------------------------------------------------------------------ reference arm
 def run_reference(args, cfg, B):
     """--impl reference: the float64 oracle as it stands, on the host cores (rank 0 only)."""
@@ -148,13 +158,15 @@ def run_reference(args, cfg, B):
         run()
     dt = time.perf_counter() - t0
     value = n * args.steps / dt
+    single = oracle_per_core(oracle, ev, pos, tilt_e, meas, geom, cores)
     sample = f"{n} positions of minibatch 0 of config {cfg.c} per step (of B={B}), float64 numpy, {cores} worker processes"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(cfg, B, extra={"sample": sample}),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "single_core": single},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -553,7 +565,8 @@ def main():
         out["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": f"{n} positions of minibatch 0 (of B={B}), forward + all gradients, float64 "
                                          f"numpy, {cores} worker processes, {dt:.1f} s (one cold call incl. process-pool "
-                                         "start-up; the --impl reference arm repeats smaller calls)"}
+                                         "start-up; the --impl reference arm repeats smaller calls)",
+                               "single_core": oracle_per_core(oracle, ev, pos, tilt_ev, meas, geom, cores)}
         # parity of the very launch shape that was timed, on the sample the oracle just computed (outside every
         # timed region): loss 1e-4, gradients 1e-3 relative L2 (BASELINE.json north_star)
         dm, dp = to(meas), to(pos)

@@ -255,8 +255,14 @@ def grad_position(obj, probe, p, tilt, a, geom, g_obj, g_probe):
     return loss_b, g_pos, g_tilt, g_dz
 
 
-def _grad_chunk(args):
-    obj, probe, positions, tilt, meas_amp, geom, idx = args
+# Inputs of the grad_batch call in flight.  Worker processes are forked AFTER this is set and read it from their copy
+# of the parent's memory, so the arrays (114 MB of complex128 object on config 4) are not pickled to every worker;
+# only the chunk's index list travels.  A parallelisation aid: no arithmetic of the method lives here.
+_SHARED = None
+
+
+def _grad_chunk(idx):
+    obj, probe, positions, tilt, meas_amp, geom = _SHARED
     Nz, H, W = obj.shape
     N = probe.shape[-1]
     r = np.floor(positions[idx] + 0.5).astype(np.int64)
@@ -287,14 +293,18 @@ def grad_batch(obj, probe, positions, tilt, meas_amp, geom, workers=1):
     tilt = np.array(_tilt_per_position(tilt, B))
     order = np.argsort(np.floor(positions[:, 0] + 0.5), kind="stable")
     workers = max(1, min(int(workers), B)) if B else 1
-    chunks = [c for c in np.array_split(order, workers) if len(c)]
-    jobs = [(obj, probe, positions, tilt, meas_amp, geom, c) for c in chunks]
-    if len(jobs) > 1:
-        import multiprocessing as mp
-        with mp.get_context("fork").Pool(len(jobs)) as pool:
-            results = pool.map(_grad_chunk, jobs)
-    else:
-        results = [_grad_chunk(j) for j in jobs]
+    global _SHARED
+    jobs = [c for c in np.array_split(order, workers) if len(c)]
+    _SHARED = (obj, probe, positions, tilt, meas_amp, geom)
+    try:
+        if len(jobs) > 1:
+            import multiprocessing as mp
+            with mp.get_context("fork").Pool(len(jobs)) as pool:      # forked here: the children see _SHARED
+                results = pool.map(_grad_chunk, jobs)
+        else:
+            results = [_grad_chunk(j) for j in jobs]
+    finally:
+        _SHARED = None
     g_object = np.zeros(obj.shape, dtype=np.complex128)
     g_probe = np.zeros(probe.shape, dtype=np.complex128)
     lb = np.zeros(B)
